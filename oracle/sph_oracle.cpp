@@ -1,0 +1,547 @@
+// oracle/sph_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, single-threaded, fp64 restatement of what the SPH hot path of arXiv:2503.09713 ("The SHAMROCK
+// code: I - SPH on GPUs", /root/reference/PAPER.md) computes. It exists only so that tests/, smoke() and
+// bench.py's cpu_baseline / --impl reference legs can check and time the CUDA path against it. It shares no
+// code with paper_2503_09713_b200/csrc and nothing in the product may call it.
+//
+// Build: g++ -std=c++17 -O2 -ffp-contract=off -fPIC -shared (see oracle/__init__.py). No FMA contraction, no
+// fast-math, no threads. Every function cites the passage of PAPER.md it follows; where the paper is silent
+// or garbled the reading of SURVEY.md 8(c) / DESIGN.md "Readings" (A1..A14, G1, G2) is taken and named.
+//
+// Parity pins (tests/test_oracle_*.py, -m "not gpu"): every function below is pinned by something other than
+// itself -- worked examples printed in the paper (delta/prefix example PAPER.md:833-869, Table B2
+// PAPER.md:899-907), brute force, closed forms (int W dV = 1, W(0) = 1/(pi h^3)), the unique-root bisection
+// for h, conservation identities (sum m a = 0, sum m (v.a + du/dt) = 0), Galilean invariance, the exact
+// Riemann solution for the Sod tube. "parity unpinned": none.
+//
+// Layout convention: vectors are SoA, pos = x[0..N) y[0..N) z[0..N) contiguous (3N doubles).
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <numeric>
+#include <vector>
+
+extern "C" {
+
+struct orc_box {
+    double lo[3], hi[3];
+    int32_t periodic[3];
+};
+
+struct orc_params {
+    double hfact;      // PAPER.md:1237 (h_fact = 1.2 for M4)
+    double gamma;      // adiabatic index, P = (gamma-1) rho u
+    double chi;        // tolerance 1.1
+    double lambda;     // Newton clamp 1.2
+    double eps_h;      // 1e-6 (north_star; eps_C not given)
+    double alpha_av;   // constant alpha (reading A10)
+    double beta_av;    // beta = 2
+    double beta_u;     // conductivity
+    double c_cour;     // 0.3
+    double c_force;    // 0.25
+    int32_t max_h_iter;
+    int32_t max_restarts;
+    int32_t eos;       // 0 adiabatic, 1 locally isothermal cs = cs0 (R/r0)^-q (BASELINE config 3)
+    int32_t newton_literal;  // reading A5: 0 = exact derivative (3 rho(h)/h), 1 = Alg. 7 line 9 as printed
+    double cs0, r0, q;
+    double GM, soft;   // fixed softened point mass (BASELINE config 3); GM = 0 disables
+    double centre[3];
+};
+
+}  // extern "C"
+
+namespace {
+
+constexpr double kRkern = 2.0;                       // M4 support radius in units of h
+constexpr double kCnorm = 0.31830988618379067154;    // 1/pi, 3-D M4 normalisation (reading O6)
+
+// ---- O6: M4 cubic B-spline (Schoenberg 1946; the paper names M4, but prints neither f nor
+// C_norm: textbook form). q = r/h.
+inline double f_m4(double q) {
+    if (q < 1.0) return 1.0 - 1.5 * q * q + 0.75 * q * q * q;
+    if (q < 2.0) { double t = 2.0 - q; return 0.25 * t * t * t; }
+    return 0.0;
+}
+inline double df_m4(double q) {
+    if (q < 1.0) return -3.0 * q + 2.25 * q * q;
+    if (q < 2.0) { double t = 2.0 - q; return -0.75 * t * t; }
+    return 0.0;
+}
+// W = C h^-3 f(q)   (Eq. 2)
+inline double W(double r, double h) { return kCnorm / (h * h * h) * f_m4(r / h); }
+// F_ab(h) = r_hat . grad_a W = C h^-4 f'(q)   (Eq. 10)
+inline double Fab(double r, double h) { return kCnorm / (h * h * h * h) * df_m4(r / h); }
+// dW/dh = -C h^-4 [3 f(q) + q f'(q)]
+inline double dWdh(double r, double h) {
+    double q = r / h;
+    return -kCnorm / (h * h * h * h) * (3.0 * f_m4(q) + q * df_m4(q));
+}
+
+// ---- minimum-image separation (reading A4): positions are kept wrapped into [lo,hi).
+inline double min_image(double d, double L, int periodic) {
+    if (periodic) {
+        if (d > 0.5 * L) d -= L;
+        else if (d < -0.5 * L) d += L;
+    }
+    return d;
+}
+
+struct Sep { double dx, dy, dz, d2; };
+inline Sep separation(const double* x, const double* y, const double* z, int64_t a, int64_t b,
+                      const orc_box& box) {
+    Sep s;
+    s.dx = min_image(x[a] - x[b], box.hi[0] - box.lo[0], box.periodic[0]);
+    s.dy = min_image(y[a] - y[b], box.hi[1] - box.lo[1], box.periodic[1]);
+    s.dz = min_image(z[a] - z[b], box.hi[2] - box.lo[2], box.periodic[2]);
+    s.d2 = s.dx * s.dx + s.dy * s.dy + s.dz * s.dz;
+    return s;
+}
+
+// gamma_o/o with the cache tolerance chi (App. E summary PAPER.md:1221; reading A2): strict <, self included.
+inline bool interacts(double d2, double ha, double hb, double chi) {
+    double rc = (kRkern * chi) * std::max(ha, hb);
+    return d2 < rc * rc;
+}
+
+inline int clz64(uint64_t v) { return v ? __builtin_clzll(v) : 64; }
+inline int clz32(uint32_t v) { return v ? __builtin_clz(v) : 32; }
+
+// delta operator (Eq. B2) on the sorted list, with Karras' index tie-break for equal keys
+// (reading O3): common-prefix length of the 96-bit strings (key, index).
+inline int delta_idx(const uint64_t* k, int64_t i, int64_t j) {
+    if (k[i] != k[j]) return clz64(k[i] ^ k[j]);
+    return 64 + clz32((uint32_t)i ^ (uint32_t)j);
+}
+
+struct TreeOut {
+    int32_t *left, *right;
+    uint8_t *lflag, *rflag;
+    int32_t *parent;   // [0,N-1): parent of internal node; [N-1, 2N-1): parent of leaf j at N-1+j; root: -1
+    int32_t *rlo, *rhi;
+};
+
+// O3: radix tree from its recursive definition: the node covering the sorted range [i,j]
+// splits where the first differing bit between its end keys changes; index convention of Table B2.
+void build_node(const uint64_t* k, int64_t N, int64_t i, int64_t j, int32_t self, int32_t parent, TreeOut& t) {
+    int d = delta_idx(k, i, j);
+    // split: last index g in [i,j) whose key shares more than d leading bits with key_i
+    int64_t g = i;
+    for (int64_t s = i + 1; s < j; ++s)
+        if (delta_idx(k, i, s) > d) g = s;
+    t.rlo[self] = (int32_t)i;
+    t.rhi[self] = (int32_t)j;
+    t.parent[self] = parent;
+    t.left[self] = (int32_t)g;
+    t.right[self] = (int32_t)(g + 1);
+    t.lflag[self] = (g == i);
+    t.rflag[self] = (g + 1 == j);
+    if (g == i) t.parent[N - 1 + g] = self; else build_node(k, N, i, g, (int32_t)g, self, t);
+    if (g + 1 == j) t.parent[N - 1 + g + 1] = self; else build_node(k, N, g + 1, j, (int32_t)(g + 1), self, t);
+}
+
+struct Box6 { double lo[3], hi[3]; double hmax; };
+
+Box6 node_box(int32_t node, bool leaf, const TreeOut& t, const double* x, const double* y, const double* z,
+              const double* h, double* aabb, double* hmax) {
+    Box6 b;
+    if (leaf) {
+        b.lo[0] = b.hi[0] = x[node]; b.lo[1] = b.hi[1] = y[node]; b.lo[2] = b.hi[2] = z[node];
+        b.hmax = h[node];
+        return b;
+    }
+    Box6 l = node_box(t.left[node], t.lflag[node], t, x, y, z, h, aabb, hmax);
+    Box6 r = node_box(t.right[node], t.rflag[node], t, x, y, z, h, aabb, hmax);
+    for (int c = 0; c < 3; ++c) { b.lo[c] = std::min(l.lo[c], r.lo[c]); b.hi[c] = std::max(l.hi[c], r.hi[c]); }
+    b.hmax = std::max(l.hmax, r.hmax);
+    for (int c = 0; c < 3; ++c) { aabb[6 * (int64_t)node + c] = b.lo[c]; aabb[6 * (int64_t)node + 3 + c] = b.hi[c]; }
+    hmax[node] = b.hmax;
+    return b;
+}
+
+// EOS (O8): adiabatic P = (gamma-1) rho u, cs = sqrt(gamma P / rho); locally isothermal P = cs(R)^2 rho.
+inline void eos(const orc_params& p, double rho, double u, double x, double y, double& P, double& cs) {
+    if (p.eos == 0) {
+        P = (p.gamma - 1.0) * rho * u;
+        cs = std::sqrt(p.gamma * P / rho);
+    } else {
+        double dx = x - p.centre[0], dy = y - p.centre[1];
+        double R = std::sqrt(dx * dx + dy * dy);
+        cs = p.cs0 * std::pow(R / p.r0, -p.q);
+        P = cs * cs * rho;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+// ---- exported scalar kernel functions (pins: quadrature, continuity, W(0)) ----
+double orc_f(double q) { return f_m4(q); }
+double orc_df(double q) { return df_m4(q); }
+double orc_W(double r, double h) { return W(r, h); }
+double orc_F(double r, double h) { return Fab(r, h); }
+double orc_dWdh(double r, double h) { return dWdh(r, h); }
+
+// ---- O1: Morton keys (grid 2^21 per axis PAPER.md:582; cube embedding, reading A1).
+// key bit (62-3j) = X bit (20-j), (61-3j) = Y, (60-3j) = Z, bit 63 = 0.
+void orc_morton_keys(int64_t N, const double* pos, const orc_box* box, uint64_t* key) {
+    double Lc = 0.0;
+    for (int c = 0; c < 3; ++c) Lc = std::max(Lc, box->hi[c] - box->lo[c]);
+    for (int64_t i = 0; i < N; ++i) {
+        uint64_t X[3];
+        for (int c = 0; c < 3; ++c) {
+            double t = (pos[c * N + i] - box->lo[c]) / Lc;
+            uint64_t v = 0;
+            if (t > 0.0) {
+                double g = std::floor(t * 2097152.0);
+                v = (g >= 2097151.0) ? 2097151u : (uint64_t)g;
+            }
+            X[c] = v;
+        }
+        uint64_t m = 0;
+        for (int j = 0; j < 21; ++j)      // j = 0 is the most significant coordinate bit (X0 of PAPER.md:827)
+            for (int c = 0; c < 3; ++c) {
+                uint64_t bit = (X[c] >> (20 - j)) & 1u;
+                m |= bit << (62 - 3 * j - c);
+            }
+        key[i] = m;
+    }
+}
+
+// worked example of PAPER.md:857-869 on beta-bit codes: delta, mask u << (beta - delta), prefix = a & mask.
+int32_t orc_delta_beta(uint64_t a, uint64_t b, int32_t beta) {
+    uint64_t xr = a ^ b;
+    if (xr == 0) return beta;
+    return clz64(xr) - (64 - beta);
+}
+uint64_t orc_prefix_mask(uint64_t a, uint64_t b, int32_t beta) {
+    uint64_t u = (beta == 64) ? ~0ull : ((1ull << beta) - 1ull);
+    int s = beta - orc_delta_beta(a, b, beta);
+    return (s >= 64) ? 0 : ((u << s) & u);
+}
+
+// ---- O2: sort by key: stable => ties by ascending input index.
+void orc_sort(int64_t N, const uint64_t* key, uint32_t* perm, uint64_t* sorted_key) {
+    std::vector<uint32_t> p(N);
+    std::iota(p.begin(), p.end(), 0u);
+    std::stable_sort(p.begin(), p.end(), [&](uint32_t a, uint32_t b) { return key[a] < key[b]; });
+    for (int64_t i = 0; i < N; ++i) { perm[i] = p[i]; sorted_key[i] = key[p[i]]; }
+}
+
+// ---- O3: radix tree tables (Table B2). Arrays of N-1 internal nodes; parent has 2N-1.
+void orc_tree(int64_t N, const uint64_t* skey, int32_t* left, int32_t* right, uint8_t* lflag, uint8_t* rflag,
+              int32_t* parent, int32_t* rlo, int32_t* rhi) {
+    if (N < 2) { if (N == 1) parent[0] = -1; return; }
+    TreeOut t{left, right, lflag, rflag, parent, rlo, rhi};
+    build_node(skey, N, 0, N - 1, 0, -1, t);
+}
+
+// ---- O4: node boxes and hmax (tight boxes, PAPER.md:93 for hmax; north_star (3)). aabb: 6 per internal node
+// (xmin,ymin,zmin,xmax,ymax,zmax); x,y,z,h in sorted order.
+void orc_aabb(int64_t N, const int32_t* left, const int32_t* right, const uint8_t* lflag, const uint8_t* rflag,
+              const double* x, const double* y, const double* z, const double* h, double* aabb, double* hmax) {
+    if (N < 2) return;
+    TreeOut t{(int32_t*)left, (int32_t*)right, (uint8_t*)lflag, (uint8_t*)rflag, nullptr, nullptr, nullptr};
+    node_box(0, false, t, x, y, z, h, aabb, hmax);
+}
+
+// ---- O5: neighbour sets, plain definition, O(N^2). CSR, each list ascending. Returns the total; fills idx
+// only if cap >= total.
+int64_t orc_neighbours_brute(int64_t N, const double* pos, const double* h, const orc_box* box, double chi,
+                             uint64_t* offs, uint32_t* idx, int64_t cap) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    int64_t total = 0;
+    for (int64_t a = 0; a < N; ++a) {
+        offs[a] = (uint64_t)total;
+        for (int64_t b = 0; b < N; ++b) {
+            Sep s = separation(x, y, z, a, b, *box);
+            if (interacts(s.d2, h[a], h[b], chi)) {
+                if (total < cap) idx[total] = (uint32_t)b;
+                ++total;
+            }
+        }
+    }
+    offs[N] = (uint64_t)total;
+    return total;
+}
+
+// Same sets through a uniform cell grid (validated against brute force in tests). For each a the grid gives
+// G(a) = {b : d^2 < (R chi h_a)^2}; N(a) = G(a) U {b : a in G(b)} because (R chi max(ha,hb))^2 =
+// max((R chi ha)^2, (R chi hb)^2) in floating point (squaring is monotone).
+int64_t orc_neighbours_grid(int64_t N, const double* pos, const double* h, const orc_box* box, double chi,
+                            uint64_t* offs, uint32_t* idx, int64_t cap) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    const double* P[3] = {x, y, z};
+    double lo[3], L[3];
+    for (int c = 0; c < 3; ++c) {
+        if (box->periodic[c]) { lo[c] = box->lo[c]; L[c] = box->hi[c] - box->lo[c]; }
+        else {
+            double mn = std::numeric_limits<double>::infinity(), mx = -mn;
+            for (int64_t i = 0; i < N; ++i) { mn = std::min(mn, P[c][i]); mx = std::max(mx, P[c][i]); }
+            lo[c] = mn; L[c] = std::max(mx - mn, 1e-300) * (1.0 + 1e-9);
+        }
+    }
+    // cell size ~ twice the median search radius, at most 128 cells per axis and at least 1
+    std::vector<double> hs(h, h + N);
+    std::nth_element(hs.begin(), hs.begin() + N / 2, hs.end());
+    double cell = std::max(2.0 * kRkern * chi * hs[N / 2], 1e-300);
+    int nc[3];
+    for (int c = 0; c < 3; ++c) nc[c] = (int)std::min(128.0, std::max(1.0, std::floor(L[c] / cell)));
+    auto cell_of = [&](int c, double v) {
+        int k = (int)std::floor((v - lo[c]) / L[c] * nc[c]);
+        return std::min(std::max(k, 0), nc[c] - 1);
+    };
+    int64_t ncell = (int64_t)nc[0] * nc[1] * nc[2];
+    std::vector<int64_t> start(ncell + 1, 0);
+    std::vector<int64_t> cid(N);
+    for (int64_t i = 0; i < N; ++i) {
+        cid[i] = ((int64_t)cell_of(0, x[i]) * nc[1] + cell_of(1, y[i])) * nc[2] + cell_of(2, z[i]);
+        ++start[cid[i] + 1];
+    }
+    for (int64_t c = 0; c < ncell; ++c) start[c + 1] += start[c];
+    std::vector<uint32_t> order(N);
+    { std::vector<int64_t> fill(start.begin(), start.end() - 1);
+      for (int64_t i = 0; i < N; ++i) order[fill[cid[i]]++] = (uint32_t)i; }
+
+    std::vector<std::vector<uint32_t>> lists(N);
+    std::vector<int> cells[3];
+    for (int64_t a = 0; a < N; ++a) {
+        double ra = kRkern * chi * h[a];
+        const double pa[3] = {x[a], y[a], z[a]};
+        for (int c = 0; c < 3; ++c) {
+            cells[c].clear();
+            double w = L[c] / nc[c];
+            int k0 = (int)std::floor((pa[c] - ra - lo[c]) / w) - 1;   // one spare cell each side
+            int k1 = (int)std::floor((pa[c] + ra - lo[c]) / w) + 1;
+            if (k1 - k0 + 1 >= nc[c]) { for (int k = 0; k < nc[c]; ++k) cells[c].push_back(k); }
+            else for (int k = k0; k <= k1; ++k) {
+                if (box->periodic[c]) cells[c].push_back(((k % nc[c]) + nc[c]) % nc[c]);
+                else if (k >= 0 && k < nc[c]) cells[c].push_back(k);
+            }
+        }
+        for (int i : cells[0]) for (int j : cells[1]) for (int k : cells[2]) {
+            int64_t c = ((int64_t)i * nc[1] + j) * nc[2] + k;
+            for (int64_t s = start[c]; s < start[c + 1]; ++s) {
+                uint32_t b = order[s];
+                Sep sp = separation(x, y, z, a, b, *box);
+                if (sp.d2 < ra * ra) {                     // b in G(a)
+                    lists[a].push_back(b);
+                    if ((int64_t)b != a && !(sp.d2 < (kRkern * chi * h[b]) * (kRkern * chi * h[b])))
+                        lists[b].push_back((uint32_t)a);   // a enters N(b) only through h_a
+                }
+            }
+        }
+    }
+    int64_t total = 0;
+    for (int64_t a = 0; a < N; ++a) {
+        auto& l = lists[a];
+        std::sort(l.begin(), l.end());
+        l.erase(std::unique(l.begin(), l.end()), l.end());
+        offs[a] = (uint64_t)total;
+        for (uint32_t b : l) { if (total < cap) idx[total] = b; ++total; }
+    }
+    offs[N] = (uint64_t)total;
+    return total;
+}
+
+// ---- O7: one pass of Alg. 7's inner loop for every particle over a given cache built
+// with h^n = hn; per-particle stopping (reading A7); safeguard 2b (reading A5b). Then rho = m (hfact/h)^3
+// (F1) and Omega (Eq. 7) at the final h. Returns the number of particles
+// that exceeded chi h^n (eps = -1 in Alg. 7 l.15-17); -1 if max_h_iter was hit.
+int64_t orc_density(int64_t N, const double* pos, const double* m, const double* hn, const uint64_t* offs,
+                    const uint32_t* idx, const orc_box* box, const orc_params* p, double* h_out,
+                    double* rho_out, double* omega_out, int32_t* iters_out, uint8_t* exceeded_out) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    int64_t n_exc = 0;
+    bool noconv = false;
+    for (int64_t a = 0; a < N; ++a) {
+        double h = hn[a];
+        bool exceeded = false, converged = false;
+        int it = 0;
+        auto sums = [&](double hh, double& rho_sum, double& S) {
+            rho_sum = 0.0; S = 0.0;
+            for (uint64_t s = offs[a]; s < offs[a + 1]; ++s) {
+                uint32_t b = idx[s];
+                double r = std::sqrt(separation(x, y, z, a, b, *box).d2);
+                rho_sum += m[b] * W(r, hh);          // Eq. 1
+                S += m[b] * dWdh(r, hh);
+            }
+        };
+        while (it < p->max_h_iter) {
+            ++it;
+            double rho_sum, S;
+            sums(h, rho_sum, S);
+            double rho_h = m[a] * (p->hfact / h) * (p->hfact / h) * (p->hfact / h);   // F1
+            double f = rho_sum - rho_h;                                               // F2
+            double fp = S + 3.0 * (p->newton_literal ? rho_sum : rho_h) / h;          // Alg. 7 l.9 / A5
+            double hnew = h - f / fp;                                                 // Alg. 7 l.10
+            if (!(fp > 0.0) || (hnew - h) * f > 0.0 || !(hnew == hnew))               // 2b safeguard
+                hnew = (f > 0.0) ? h / p->lambda : h * p->lambda;
+            if (hnew > h * p->lambda) hnew = h * p->lambda;                           // Alg. 7 l.11-13
+            else if (hnew < h / p->lambda) hnew = h / p->lambda;
+            double eps = std::fabs(hnew - h) / hn[a];                                 // Alg. 7 l.14
+            if (hnew > hn[a] * p->chi) { hnew = hn[a] * p->chi; exceeded = true; }    // Alg. 7 l.15-17
+            h = hnew;
+            if (exceeded) break;
+            if (eps <= p->eps_h) { converged = true; break; }
+        }
+        if (!exceeded && !converged) noconv = true;
+        double rho_sum, S;
+        sums(h, rho_sum, S);
+        double rho = m[a] * (p->hfact / h) * (p->hfact / h) * (p->hfact / h);
+        h_out[a] = h;
+        rho_out[a] = rho;
+        omega_out[a] = 1.0 + h / (3.0 * rho) * S;    // Eq. 7 with dh/drho = -h/(3 rho) from F1
+        if (iters_out) iters_out[a] = it;
+        if (exceeded_out) exceeded_out[a] = exceeded;
+        n_exc += exceeded;
+    }
+    return noconv ? -1 : n_exc;
+}
+
+// Pin for O7: h_a as the unique root of g_a(h) = sum_b m_b C f(r_ab/h) - m_a hfact^3 (reading A5b), found by
+// plain bisection over ALL particles (no cache, no Newton).
+void orc_h_bisect(int64_t N, const double* pos, const double* m, const orc_box* box, double hfact,
+                  const double* h_lo, const double* h_hi, double* h_out) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    std::vector<double> r(N);
+    for (int64_t a = 0; a < N; ++a) {
+        for (int64_t b = 0; b < N; ++b) r[b] = std::sqrt(separation(x, y, z, a, b, *box).d2);
+        auto g = [&](double h) {
+            double s = 0.0;
+            for (int64_t b = 0; b < N; ++b) s += m[b] * kCnorm * f_m4(r[b] / h);
+            return s - m[a] * hfact * hfact * hfact;
+        };
+        double lo = h_lo[a], hi = h_hi[a];
+        for (int it = 0; it < 200; ++it) {
+            double mid = 0.5 * (lo + hi);
+            if (mid == lo || mid == hi) break;
+            if (g(mid) > 0.0) hi = mid; else lo = mid;
+        }
+        h_out[a] = 0.5 * (lo + hi);
+    }
+}
+
+// ---- O8 + O9: forces (Eq. 3-6, 8-10; minus sign G1, q inside the sum G2), per-particle CFL
+// candidates (G8; v_sig^dt reading A12) and their global minimum.
+double orc_forces(int64_t N, const double* pos, const double* vel, const double* m, const double* h,
+                  const double* rho, const double* omega, const double* u, const uint64_t* offs,
+                  const uint32_t* idx, const orc_box* box, const orc_params* p, double* acc, double* dudt) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    const double *vx = vel, *vy = vel + N, *vz = vel + 2 * N;
+    std::vector<double> P(N), cs(N);
+    for (int64_t a = 0; a < N; ++a) eos(*p, rho[a], u[a], x[a], y[a], P[a], cs[a]);
+    double dt_min = std::numeric_limits<double>::infinity();
+    for (int64_t a = 0; a < N; ++a) {
+        double ax = 0.0, ay = 0.0, az = 0.0, du = 0.0;
+        double vsig_dt = cs[a];
+        for (uint64_t s = offs[a]; s < offs[a + 1]; ++s) {
+            uint32_t b = idx[s];
+            if ((int64_t)b == a) continue;
+            Sep sp = separation(x, y, z, a, b, *box);
+            double r = std::sqrt(sp.d2);
+            if (!(r > 0.0)) continue;                       // coincident particles: r_hat undefined
+            double rx = sp.dx / r, ry = sp.dy / r, rz = sp.dz / r;
+            double dvx = vx[a] - vx[b], dvy = vy[a] - vy[b], dvz = vz[a] - vz[b];
+            double w = dvx * rx + dvy * ry + dvz * rz;      // v_ab . r_hat_ab
+            double vsa = p->alpha_av * cs[a] + p->beta_av * std::fabs(w);   // Eq. 6
+            double vsb = p->alpha_av * cs[b] + p->beta_av * std::fabs(w);
+            double qa = (w < 0.0) ? -0.5 * rho[a] * vsa * w : 0.0;          // Eq. 5
+            double qb = (w < 0.0) ? -0.5 * rho[b] * vsb * w : 0.0;
+            double Fa = Fab(r, h[a]), Fb = Fab(r, h[b]);                    // Eq. 10
+            double ta = (P[a] + qa) / (rho[a] * rho[a] * omega[a]);
+            double tb = (P[b] + qb) / (rho[b] * rho[b] * omega[b]);
+            double coef = m[b] * (ta * Fa + tb * Fb);
+            ax -= coef * rx; ay -= coef * ry; az -= coef * rz;              // Eq. 3 (with G1's minus sign)
+            du += m[b] * ta * w * Fa;                                       // Eq. 4 (G2: inside the sum)
+            if (p->eos == 0 && p->beta_u != 0.0) {
+                double vsu = std::sqrt(std::fabs(P[a] - P[b]) / (0.5 * (rho[a] + rho[b])));   // Eq. 9
+                du += m[b] * p->beta_u * vsu * (u[a] - u[b]) * 0.5 *
+                      (Fa / (omega[a] * rho[a]) + Fb / (omega[b] * rho[b]));                  // Eq. 8
+            }
+            if (r < kRkern * std::max(h[a], h[b])) vsig_dt = std::max(vsig_dt, vsa);           // A12
+        }
+        if (p->GM != 0.0) {                                 // fixed softened point mass (config 3)
+            double dx = x[a] - p->centre[0], dy = y[a] - p->centre[1], dz = z[a] - p->centre[2];
+            double d2 = dx * dx + dy * dy + dz * dz + p->soft * p->soft;
+            double inv = p->GM / (d2 * std::sqrt(d2));
+            ax -= inv * dx; ay -= inv * dy; az -= inv * dz;
+        }
+        if (p->eos != 0) du = 0.0;
+        acc[a] = ax; acc[N + a] = ay; acc[2 * N + a] = az;
+        dudt[a] = du;
+        double an = std::sqrt(ax * ax + ay * ay + az * az);
+        double dta = p->c_cour * h[a] / vsig_dt;                            // G8
+        if (an > 0.0) dta = std::min(dta, p->c_force * std::sqrt(h[a] / an));
+        dt_min = std::min(dt_min, dta);
+    }
+    return dt_min;
+}
+
+// ---- single evaluation: neighbours at h^n -> Alg. 7 with chi-restarts (outer while) ->
+// forces. h is in/out (h^n in, converged h out). mode 0 = brute-force neighbour search, 1 = cell grid.
+// Returns restarts >= 0, or -1 (h iteration cap), -2 (restart cap). If offs_out/idx_out are non-null and
+// cap suffices they receive the final cache.
+int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
+                     double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
+                     double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out) {
+    std::vector<uint64_t> offs(N + 1);
+    std::vector<uint32_t> idx;
+    std::vector<double> hn(h, h + N), hnew(N);
+    int32_t restarts = 0;
+    for (;;) {
+        auto search = mode ? orc_neighbours_grid : orc_neighbours_brute;
+        int64_t total = search(N, pos, hn.data(), box, p->chi, offs.data(), nullptr, 0);
+        idx.resize(total);
+        search(N, pos, hn.data(), box, p->chi, offs.data(), idx.data(), total);
+        int64_t ne = orc_density(N, pos, m, hn.data(), offs.data(), idx.data(), box, p, hnew.data(), rho, omega,
+                                 nullptr, nullptr);
+        if (ne < 0) return -1;
+        if (ne == 0) break;
+        hn = hnew;                      // h^n <- current h for all particles, rebuild, rerun
+        if (++restarts > p->max_restarts) return -2;
+    }
+    std::memcpy(h, hnew.data(), N * sizeof(double));
+    double dt = orc_forces(N, pos, vel, m, h, rho, omega, u, offs.data(), idx.data(), box, p, acc, dudt);
+    if (dt_out) *dt_out = dt;
+    if (n_neigh_out) *n_neigh_out = (int64_t)idx.size();
+    return restarts;
+}
+
+// ---- O10: one leapfrog KDK step (G1-G5; order of Fig. G1; u integrated
+// like v, reading A13). State in/out: pos, vel, u, h, acc, dudt (a^n, du/dt^n on entry; ^{n+1} on exit).
+// Returns restarts or a negative error like orc_evaluate; dt_next receives the CFL dt for the next step (A14).
+int32_t orc_step(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                 double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                 double* omega, double* dt_next) {
+    std::vector<double> a_old(acc, acc + 3 * N), du_old(dudt, dudt + N);
+    for (int c = 0; c < 3; ++c) {
+        double L = box->hi[c] - box->lo[c];
+        for (int64_t i = 0; i < N; ++i) {
+            double vh = vel[c * N + i] + 0.5 * dt * a_old[c * N + i];        // G1
+            double r = pos[c * N + i] + dt * vh;                            // G2
+            if (box->periodic[c]) {                                         // wrap into [lo,hi)
+                if (r >= box->hi[c]) r -= L;
+                else if (r < box->lo[c]) r += L;
+                if (r >= box->hi[c]) r = box->lo[c];                        // r + L rounding up to hi
+            }
+            pos[c * N + i] = r;
+            vel[c * N + i] = vh + 0.5 * dt * a_old[c * N + i];              // G3
+        }
+    }
+    for (int64_t i = 0; i < N; ++i) {
+        double uh = u[i] + 0.5 * dt * du_old[i];
+        u[i] = uh + 0.5 * dt * du_old[i];
+    }
+    int32_t rc = orc_evaluate(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, dt_next, nullptr);   // G4
+    if (rc < 0) return rc;
+    for (int64_t i = 0; i < 3 * N; ++i) vel[i] = vel[i] + 0.5 * dt * (acc[i] - a_old[i]);                     // G5
+    for (int64_t i = 0; i < N; ++i) u[i] = u[i] + 0.5 * dt * (dudt[i] - du_old[i]);
+    return rc;
+}
+
+}  // extern "C"
