@@ -1,0 +1,533 @@
+// api.cu -- the C ABI of include/sph_b200.h: context, memory, call-order state machine, step orchestration,
+// getters/setters and per-stage CUDA-event timers. All arithmetic of the hot path lives in the kernels of the
+// sibling .cu files; there is no CPU fallback anywhere in this library.
+#include <stdarg.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "common.cuh"
+
+using namespace sph;
+
+namespace sph {
+
+int fail(sph_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static void* default_alloc(size_t bytes, void*) {
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+static void default_free(void* p, void*) { cudaFree(p); }
+
+template <typename T>
+static int dalloc(sph_ctx* c, T** out, size_t count) {
+    size_t bytes = std::max<size_t>(count * sizeof(T), 256);
+    void* p = c->alloc.alloc(bytes, c->alloc.user);
+    if (!p) return fail(c, SPH_ERR_OOM, "device allocation of %zu bytes failed", bytes);
+    c->allocations.push_back(p);
+    c->bytes_allocated += (int64_t)bytes;
+    *out = reinterpret_cast<T*>(p);
+    return SPH_OK;
+}
+static void dfree(sph_ctx* c, void* p) {
+    if (!p) return;
+    auto it = std::find(c->allocations.begin(), c->allocations.end(), p);
+    if (it != c->allocations.end()) c->allocations.erase(it);
+    c->alloc.release(p, c->alloc.user);
+}
+
+static int alloc_fields(sph_ctx* c, Fields& f) {
+    const size_t N = (size_t)c->N;
+    double *pos, *vel, *acc;
+    SPH_TRY(dalloc(c, &pos, 3 * N));   // x|y|z contiguous so that 3-component copies are one kernel
+    SPH_TRY(dalloc(c, &vel, 3 * N));
+    SPH_TRY(dalloc(c, &acc, 3 * N));
+    f.x = pos; f.y = pos + N; f.z = pos + 2 * N;
+    f.vx = vel; f.vy = vel + N; f.vz = vel + 2 * N;
+    f.ax = acc; f.ay = acc + N; f.az = acc + 2 * N;
+    SPH_TRY(dalloc(c, &f.u, N));
+    SPH_TRY(dalloc(c, &f.du, N));
+    SPH_TRY(dalloc(c, &f.h, N));
+    SPH_TRY(dalloc(c, &f.m, N));
+    SPH_TRY(dalloc(c, &f.id, N));
+    return SPH_OK;
+}
+
+// ---- timers ----
+struct StageTimer {
+    sph_ctx* c;
+    StageTimer(sph_ctx* ctx, int stage) : c(ctx) {
+        TimerRec r;
+        r.stage = stage;
+        r.e0 = get(); r.e1 = get();
+        cudaEventRecord(r.e0, c->stream);
+        c->timers.push_back(r);
+    }
+    ~StageTimer() { cudaEventRecord(c->timers.back().e1, c->stream); }
+    cudaEvent_t get() {
+        if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+        cudaEvent_t e; cudaEventCreate(&e); return e;
+    }
+};
+
+static int read_scalars(sph_ctx* c) {
+    SPH_CUDA(c, cudaMemcpyAsync(c->h_sc, c->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+__global__ void k_iota(int64_t N, uint32_t* id) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) id[i] = (uint32_t)i;
+}
+__global__ void k_fill(int64_t N, double* p, double v) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) p[i] = v;
+}
+// fallback h0 = hfact (m V / M_tot)^(1/3) (reading A9); M_tot by a simple two-kernel reduction
+__global__ void k_sum(int64_t N, const double* __restrict__ m, double* out) {
+    double v = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) v += m[i];
+    v = warp_sum(v);
+    if (lane_id() == 0) atomicAdd(out, v);
+}
+__global__ void k_h0_fallback(int64_t N, const double* __restrict__ m, const double* mtot, double vol, double hfact, double* h) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) h[i] = hfact * cbrt(m[i] * vol / *mtot);
+}
+__global__ void k_store_total(const uint64_t* offs, int64_t N, DevScalars* sc) { sc->n_neigh = offs[N]; }
+
+// neighbour cache for the current tree and h^n: hmax -> AABB -> count -> scan -> (sync) -> fill
+static int cache_build(sph_ctx* c) {
+    { StageTimer t(c, ST_AABB); SPH_TRY(launch_hmax(c)); SPH_TRY(launch_aabb(c)); }
+    { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c, false)); }
+    {
+        StageTimer t(c, ST_SCAN);
+        SPH_TRY(launch_scan_u32_u64(c, c->cnt, c->offs, c->N, nullptr));
+        k_store_total<<<1, 1, 0, c->stream>>>(c->offs, c->N, c->d_sc);
+        c->launches++;
+    }
+    SPH_TRY(read_scalars(c));
+    const DevScalars& s = *c->h_sc;
+    for (int k = 0; k < 3; ++k)
+        if (c->box.periodic[k] && !(2.0 * kRkern * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
+            return fail(c, SPH_ERR_PERIODIC_TOO_SMALL, "periodic axis %d: 2 R_kern chi h_max = %g >= L = %g", k,
+                        2.0 * kRkern * c->p.chi * s.h_max, c->box.hi[k] - c->box.lo[k]);
+    c->n_neigh = s.n_neigh;
+    c->n_groups = s.n_groups;
+    if (c->n_neigh > c->nbr_cap) {
+        dfree(c, c->nbr);
+        c->nbr = nullptr;
+        c->nbr_cap = 0;
+        uint64_t cap = c->n_neigh + c->n_neigh / 8 + 1024;
+        SPH_TRY(dalloc(c, &c->nbr, (size_t)cap));
+        c->nbr_cap = cap;
+    }
+    { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c, true)); }
+    return SPH_OK;
+}
+
+static int check_ctx(sph_ctx* c) { return c ? SPH_OK : SPH_ERR_ARG; }
+
+}  // namespace sph
+
+extern "C" {
+
+void sph_default_params(sph_params* p) {
+    if (!p) return;
+    memset(p, 0, sizeof(*p));
+    p->hfact = 1.2; p->gamma = 5.0 / 3.0; p->chi = 1.1; p->lambda = 1.2; p->eps_h = 1e-6;
+    p->alpha_av = 1.0; p->beta_av = 2.0; p->beta_u = 1.0; p->c_cour = 0.3; p->c_force = 0.25;
+    p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0;
+    p->cs0 = 1.0; p->r0 = 1.0; p->q = 0.0; p->GM = 0.0; p->soft = 0.0;
+}
+
+const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
+
+void sph_free(sph_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    for (auto& t : c->timers) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
+    for (auto e : c->event_pool) cudaEventDestroy(e);
+    std::vector<void*> all = c->allocations;
+    for (void* p : all) c->alloc.release(p, c->alloc.user);
+    if (c->h_sc) cudaFreeHost(c->h_sc);
+    delete c;
+}
+
+int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const double* vel, const double* mass,
+                const double* u, const double* h0, const sph_box* box, const sph_params* params, void* cuda_stream,
+                const sph_allocator* allocator, int run_white_step) {
+    if (!out) return SPH_ERR_ARG;
+    *out = nullptr;
+    if (N < 1 || N >= (1ll << 30) || !pos || !vel || !mass || !u || !box) return SPH_ERR_ARG;
+    for (int k = 0; k < 3; ++k)
+        if (!(box->hi[k] > box->lo[k])) return SPH_ERR_ARG;
+    int dev = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) { cudaGetLastError(); return SPH_ERR_DEVICE; }
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SPH_ERR_DEVICE;
+    if (prop.major != 10) return SPH_ERR_DEVICE;   // sm_100a code only; no fallback path exists
+
+    sph_ctx* c = new (std::nothrow) sph_ctx();
+    if (!c) return SPH_ERR_OOM;
+    *out = c;   // returned even on failure so that sph_last_error() can be read; caller frees it
+    c->N = N;
+    c->box = *box;
+    if (params) c->p = *params; else sph_default_params(&c->p);
+    if (!(c->p.hfact > 0) || !(c->p.chi >= 1.0) || !(c->p.lambda > 1.0) || !(c->p.eps_h > 0) || c->p.max_h_iter < 1)
+        return fail(c, SPH_ERR_ARG, "bad parameters");
+    c->stream = (cudaStream_t)cuda_stream;
+    if (allocator && allocator->alloc && allocator->release) c->alloc = *allocator;
+    else { c->alloc.alloc = default_alloc; c->alloc.release = default_free; c->alloc.user = nullptr; }
+
+    const size_t n = (size_t)N;
+    SPH_TRY(alloc_fields(c, c->cur));
+    SPH_TRY(alloc_fields(c, c->alt));
+    SPH_TRY(dalloc(c, &c->rho, n)); SPH_TRY(dalloc(c, &c->omega, n)); SPH_TRY(dalloc(c, &c->P, n));
+    SPH_TRY(dalloc(c, &c->cs, n)); SPH_TRY(dalloc(c, &c->A, n)); SPH_TRY(dalloc(c, &c->hnew, n));
+    SPH_TRY(dalloc(c, &c->nax, 3 * n));
+    c->nay = c->nax + n; c->naz = c->nax + 2 * n;
+    SPH_TRY(dalloc(c, &c->ndu, n));
+    SPH_TRY(dalloc(c, &c->key, n)); SPH_TRY(dalloc(c, &c->key_alt, n));
+    SPH_TRY(dalloc(c, &c->val, n)); SPH_TRY(dalloc(c, &c->val_alt, n));
+    size_t status_bytes;
+    sort_scratch_bytes(N, &c->sort_tiles, &status_bytes);
+    SPH_TRY(dalloc(c, &c->sort_hist, 8 * 256));
+    SPH_TRY(dalloc(c, &c->sort_status, status_bytes / sizeof(uint32_t)));
+    SPH_TRY(dalloc(c, &c->sort_counters, 16));
+    SPH_TRY(dalloc(c, &c->nodes, n));
+    SPH_TRY(dalloc(c, &c->parent, 2 * n));
+    SPH_TRY(dalloc(c, &c->visit, n));
+    SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
+    SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->offs, n + 1));
+    c->scan_tiles = scan_scratch_tiles(N);
+    SPH_TRY(dalloc(c, &c->scan_status, (size_t)c->scan_tiles));
+    SPH_TRY(dalloc(c, &c->scan_counter, 4));
+    SPH_TRY(dalloc(c, &c->d_sc, 1));
+    SPH_TRY(dalloc(c, &c->d_dtstep, 4));
+    SPH_CUDA(c, cudaMallocHost((void**)&c->h_sc, sizeof(DevScalars)));
+    SPH_CUDA(c, cudaMemsetAsync(c->d_sc, 0, sizeof(DevScalars), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(c->d_dtstep, 0, 4 * sizeof(double), c->stream));
+
+    // inputs, original order: slot i holds particle i, id = iota
+    const cudaMemcpyKind kind = (mem == SPH_MEM_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    SPH_CUDA(c, cudaMemcpyAsync(c->cur.x, pos, 3 * n * sizeof(double), kind, c->stream));
+    SPH_CUDA(c, cudaMemcpyAsync(c->cur.vx, vel, 3 * n * sizeof(double), kind, c->stream));
+    SPH_CUDA(c, cudaMemcpyAsync(c->cur.m, mass, n * sizeof(double), kind, c->stream));
+    SPH_CUDA(c, cudaMemcpyAsync(c->cur.u, u, n * sizeof(double), kind, c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(c->cur.ax, 0, 3 * n * sizeof(double), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(c->cur.du, 0, n * sizeof(double), c->stream));
+    k_iota<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.id);
+    c->launches++;
+    if (h0) {
+        SPH_CUDA(c, cudaMemcpyAsync(c->cur.h, h0, n * sizeof(double), kind, c->stream));
+    } else {
+        double vol = 1.0;
+        for (int k = 0; k < 3; ++k) vol *= box->hi[k] - box->lo[k];
+        double* mtot = c->d_dtstep + 1;
+        k_sum<<<(unsigned)std::min<int64_t>(592, (N + 255) / 256), 256, 0, c->stream>>>(N, c->cur.m, mtot);
+        k_h0_fallback<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, mtot, vol, c->p.hfact, c->cur.h);
+        c->launches += 2;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    c->state = S_FIELDS;
+    if (run_white_step) {
+        SPH_TRY(sph_build_tree(c));
+        SPH_TRY(sph_compute_density(c));
+        SPH_TRY(sph_compute_forces(c));
+    }
+    return SPH_OK;
+}
+
+int sph_init(sph_ctx** out, int64_t N, const double* pos_dev, const double* vel_dev, const double* mass_dev,
+             const double* u_dev, const sph_box* box, double gamma, double hfact) {
+    sph_params p;
+    sph_default_params(&p);
+    p.gamma = gamma;
+    p.hfact = hfact;
+    return sph_init_ex(out, N, SPH_MEM_DEVICE, pos_dev, vel_dev, mass_dev, u_dev, nullptr, box, &p, nullptr, nullptr, 1);
+}
+
+int sph_build_tree(sph_ctx* c) {
+    SPH_TRY(check_ctx(c));
+    { StageTimer t(c, ST_KEYS); SPH_TRY(launch_keys(c)); }
+    { StageTimer t(c, ST_SORT); SPH_TRY(launch_sort(c)); }
+    { StageTimer t(c, ST_PERMUTE); SPH_TRY(launch_permute(c)); }
+    { StageTimer t(c, ST_TREE); SPH_TRY(launch_tree(c)); }
+    SPH_TRY(cache_build(c));
+    c->state = S_TREE;
+    return SPH_OK;
+}
+
+int sph_compute_density(sph_ctx* c) {
+    SPH_TRY(check_ctx(c));
+    if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "sph_compute_density needs sph_build_tree first");
+    int restarts = 0;
+    for (;;) {
+        { StageTimer t(c, ST_DENSITY); SPH_TRY(launch_density(c)); }
+        SPH_TRY(read_scalars(c));
+        if (c->h_sc->n_noconv)
+            return fail(c, SPH_ERR_H_NOCONV, "%u particles did not converge in %d Newton iterations", c->h_sc->n_noconv,
+                        c->p.max_h_iter);
+        std::swap(c->cur.h, c->hnew);            // h^n <- h (all particles), Alg. 7 outer loop
+        if (c->h_sc->n_exceeded == 0) break;
+        if (++restarts > c->p.max_restarts)
+            return fail(c, SPH_ERR_RESTARTS, "more than %d chi-restarts (%u particles still exceed chi h^n)",
+                        c->p.max_restarts, c->h_sc->n_exceeded);
+        SPH_TRY(cache_build(c));                 // positions unchanged: same keys, order and topology; new hmax, cache
+    }
+    c->restarts_last = restarts;
+    c->state = S_DENSITY;
+    return SPH_OK;
+}
+
+static int forces_eval(sph_ctx* c) {
+    if (c->state < S_DENSITY) return fail(c, SPH_ERR_ORDER, "sph_compute_forces needs sph_compute_density first");
+    { StageTimer t(c, ST_FORCES); SPH_TRY(launch_forces(c)); }
+    c->have_cfl_dt = true;
+    c->state = S_FORCES;
+    return SPH_OK;
+}
+
+int sph_compute_forces(sph_ctx* c) {
+    SPH_TRY(check_ctx(c));
+    SPH_TRY(forces_eval(c));
+    // standalone evaluation (and the white step): the result becomes a^n, du/dt^n of the next predictor
+    StageTimer t(c, ST_LEAPFROG);
+    return launch_adopt_acc(c);
+}
+
+int sph_step_leapfrog(sph_ctx* c, double dt, double* dt_used) {
+    SPH_TRY(check_ctx(c));
+    if (!c->have_cfl_dt) return fail(c, SPH_ERR_ORDER, "sph_step_leapfrog needs a force evaluation (a^n, dt) first");
+    {
+        StageTimer t(c, ST_LEAPFROG);
+        SPH_TRY(launch_set_dt(c, dt));
+        SPH_TRY(launch_predict(c));
+    }
+    c->state = S_FIELDS;
+    SPH_TRY(sph_build_tree(c));
+    SPH_TRY(sph_compute_density(c));
+    SPH_TRY(forces_eval(c));
+    { StageTimer t(c, ST_LEAPFROG); SPH_TRY(launch_correct(c)); }
+    c->steps++;
+    if (dt_used) {
+        SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d_dtstep, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    return SPH_OK;
+}
+
+static int copy_in(sph_ctx* c, sph_mem mem, const double* src, double* dst_sorted, int ncomp, double** stage) {
+    if (!src) return SPH_OK;
+    const size_t bytes = (size_t)ncomp * c->N * sizeof(double);
+    const double* dev_src = src;
+    if (mem == SPH_MEM_HOST) {
+        if (!*stage) SPH_TRY(dalloc(c, stage, 3 * (size_t)c->N));
+        SPH_CUDA(c, cudaMemcpyAsync(*stage, src, bytes, cudaMemcpyHostToDevice, c->stream));
+        dev_src = *stage;
+    }
+    return launch_gather_orig_f64(c, dev_src, dst_sorted, ncomp);
+}
+static int copy_out(sph_ctx* c, sph_mem mem, const double* src_sorted, double* dst, int ncomp, double** stage) {
+    if (!dst) return SPH_OK;
+    const size_t bytes = (size_t)ncomp * c->N * sizeof(double);
+    if (mem == SPH_MEM_HOST) {
+        if (!*stage) SPH_TRY(dalloc(c, stage, 3 * (size_t)c->N));
+        SPH_TRY(launch_scatter_orig_f64(c, src_sorted, *stage, ncomp));
+        SPH_CUDA(c, cudaMemcpyAsync(dst, *stage, bytes, cudaMemcpyDeviceToHost, c->stream));
+        return SPH_OK;
+    }
+    return launch_scatter_orig_f64(c, src_sorted, dst, ncomp);
+}
+
+int sph_set_fields(sph_ctx* c, sph_mem mem, const double* pos, const double* vel, const double* u, const double* h,
+                   const double* acc, const double* dudt) {
+    SPH_TRY(check_ctx(c));
+    double* stage = nullptr;   // one staging buffer reused in stream order
+    int rc = SPH_OK;
+    if ((rc = copy_in(c, mem, pos, c->cur.x, 3, &stage)) == SPH_OK && (rc = copy_in(c, mem, vel, c->cur.vx, 3, &stage)) == SPH_OK &&
+        (rc = copy_in(c, mem, u, c->cur.u, 1, &stage)) == SPH_OK && (rc = copy_in(c, mem, h, c->cur.h, 1, &stage)) == SPH_OK &&
+        (rc = copy_in(c, mem, acc, c->cur.ax, 3, &stage)) == SPH_OK)
+        rc = copy_in(c, mem, dudt, c->cur.du, 1, &stage);
+    if (stage) { cudaStreamSynchronize(c->stream); dfree(c, stage); }
+    if (rc != SPH_OK) return rc;
+    if (pos || vel || u || h) c->state = S_FIELDS;
+    return SPH_OK;
+}
+
+int sph_get_fields(sph_ctx* c, sph_mem mem, double* pos, double* vel, double* u, double* h, double* rho, double* omega,
+                   double* acc, double* dudt) {
+    SPH_TRY(check_ctx(c));
+    if ((rho || omega) && c->state < S_DENSITY) return fail(c, SPH_ERR_ORDER, "rho/omega need sph_compute_density");
+    double* stage = nullptr;
+    int rc = SPH_OK;
+    // with a host destination each field goes through the staging buffer; the D2H copy is stream-ordered
+    // after its scatter and before the next scatter overwrites the buffer
+    if ((rc = copy_out(c, mem, c->cur.x, pos, 3, &stage)) == SPH_OK && (rc = copy_out(c, mem, c->cur.vx, vel, 3, &stage)) == SPH_OK &&
+        (rc = copy_out(c, mem, c->cur.u, u, 1, &stage)) == SPH_OK && (rc = copy_out(c, mem, c->cur.h, h, 1, &stage)) == SPH_OK &&
+        (rc = copy_out(c, mem, c->rho, rho, 1, &stage)) == SPH_OK && (rc = copy_out(c, mem, c->omega, omega, 1, &stage)) == SPH_OK &&
+        (rc = copy_out(c, mem, c->cur.ax, acc, 3, &stage)) == SPH_OK)
+        rc = copy_out(c, mem, c->cur.du, dudt, 1, &stage);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (stage) dfree(c, stage);
+    if (rc != SPH_OK) return rc;
+    if (e != cudaSuccess) return fail(c, SPH_ERR_DEVICE, "stream sync failed: %s", cudaGetErrorString(e));
+    return SPH_OK;
+}
+
+static int copy_raw(sph_ctx* c, sph_mem mem, void* dst, const void* src_dev, size_t bytes) {
+    if (!dst || bytes == 0) return SPH_OK;
+    SPH_CUDA(c, cudaMemcpyAsync(dst, src_dev, bytes, mem == SPH_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
+                                c->stream));
+    return SPH_OK;
+}
+
+int sph_get_keys_perm(sph_ctx* c, sph_mem mem, uint64_t* sorted_keys, uint32_t* perm) {
+    SPH_TRY(check_ctx(c));
+    if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no tree built");
+    SPH_TRY(copy_raw(c, mem, sorted_keys, c->key, (size_t)c->N * sizeof(uint64_t)));
+    SPH_TRY(copy_raw(c, mem, perm, c->cur.id, (size_t)c->N * sizeof(uint32_t)));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+__global__ void k_export_tree(int64_t N, const NodeRec* __restrict__ nodes, int32_t* left, int32_t* right, uint8_t* lflag,
+                              uint8_t* rflag, int32_t* rlo, int32_t* rhi, double* aabb, double* hmax) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N - 1) return;
+    const NodeRec r = nodes[i];
+    const int32_t lo = min((int32_t)i, r.other), hi = max((int32_t)i, r.other);
+    if (left) left[i] = r.split;
+    if (right) right[i] = r.split + 1;
+    if (lflag) lflag[i] = (lo == r.split);
+    if (rflag) rflag[i] = (hi == r.split + 1);
+    if (rlo) rlo[i] = lo;
+    if (rhi) rhi[i] = hi;
+    if (aabb) for (int k = 0; k < 3; ++k) { aabb[6 * i + k] = r.lo[k]; aabb[6 * i + 3 + k] = r.hi[k]; }
+    if (hmax) hmax[i] = r.hmax;
+}
+
+int sph_get_tree(sph_ctx* c, sph_mem mem, int32_t* left, int32_t* right, uint8_t* lflag, uint8_t* rflag, int32_t* parent,
+                 int32_t* range_lo, int32_t* range_hi, double* aabb, double* hmax) {
+    SPH_TRY(check_ctx(c));
+    if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no tree built");
+    const int64_t N = c->N, ni = N - 1;
+    if (parent) {
+        if (N == 1) { int32_t m1 = -1; SPH_CUDA(c, cudaMemcpyAsync(c->parent, &m1, 4, cudaMemcpyHostToDevice, c->stream)); }
+        SPH_TRY(copy_raw(c, mem, parent, c->parent, (size_t)(2 * N - 1) * sizeof(int32_t)));
+    }
+    if (ni < 1) { SPH_CUDA(c, cudaStreamSynchronize(c->stream)); return SPH_OK; }
+    // export through device temporaries (debug path), then copy to the caller's memory
+    int32_t *t_i = nullptr; uint8_t* t_b = nullptr; double* t_d = nullptr;
+    SPH_TRY(dalloc(c, &t_i, 4 * (size_t)ni));
+    SPH_TRY(dalloc(c, &t_b, 2 * (size_t)ni));
+    SPH_TRY(dalloc(c, &t_d, 7 * (size_t)ni));
+    k_export_tree<<<div_up(ni, 256), 256, 0, c->stream>>>(N, c->nodes, t_i, t_i + ni, t_b, t_b + ni, t_i + 2 * ni, t_i + 3 * ni,
+                                                          t_d, t_d + 6 * ni);
+    c->launches++;
+    int rc = SPH_OK;
+    if ((rc = copy_raw(c, mem, left, t_i, ni * 4)) == SPH_OK && (rc = copy_raw(c, mem, right, t_i + ni, ni * 4)) == SPH_OK &&
+        (rc = copy_raw(c, mem, lflag, t_b, ni)) == SPH_OK && (rc = copy_raw(c, mem, rflag, t_b + ni, ni)) == SPH_OK &&
+        (rc = copy_raw(c, mem, range_lo, t_i + 2 * ni, ni * 4)) == SPH_OK &&
+        (rc = copy_raw(c, mem, range_hi, t_i + 3 * ni, ni * 4)) == SPH_OK && (rc = copy_raw(c, mem, aabb, t_d, 6 * ni * 8)) == SPH_OK)
+        rc = copy_raw(c, mem, hmax, t_d + 6 * ni, ni * 8);
+    cudaStreamSynchronize(c->stream);
+    dfree(c, t_i); dfree(c, t_b); dfree(c, t_d);
+    return rc;
+}
+
+int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
+    SPH_TRY(check_ctx(c));
+    if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no neighbour cache built");
+    SPH_TRY(copy_raw(c, mem, offs, c->offs, (size_t)(c->N + 1) * sizeof(uint64_t)));
+    if (idx) {
+        if (cap < c->n_neigh) return fail(c, SPH_ERR_CAP, "idx capacity %llu < %llu neighbours", (unsigned long long)cap,
+                                          (unsigned long long)c->n_neigh);
+        SPH_TRY(copy_raw(c, mem, idx, c->nbr, (size_t)c->n_neigh * sizeof(uint32_t)));
+    }
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+int sph_reset_timers(sph_ctx* c) {
+    SPH_TRY(check_ctx(c));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (auto& t : c->timers) { c->event_pool.push_back(t.e0); c->event_pool.push_back(t.e1); }
+    c->timers.clear();
+    c->launches = 0;
+    return SPH_OK;
+}
+
+int sph_get_stats(sph_ctx* c, sph_stats* out) {
+    SPH_TRY(check_ctx(c));
+    if (!out) return SPH_ERR_ARG;
+    memset(out, 0, sizeof(*out));
+    SPH_TRY(read_scalars(c));
+    double ms[ST_COUNT] = {0};
+    for (auto& t : c->timers) {
+        float v = 0.f;
+        if (cudaEventElapsedTime(&v, t.e0, t.e1) == cudaSuccess) ms[t.stage] += v; else cudaGetLastError();
+    }
+    out->ms_keys = ms[ST_KEYS]; out->ms_sort = ms[ST_SORT]; out->ms_permute = ms[ST_PERMUTE]; out->ms_tree = ms[ST_TREE];
+    out->ms_aabb = ms[ST_AABB]; out->ms_traverse = ms[ST_TRAVERSE]; out->ms_scan = ms[ST_SCAN];
+    out->ms_density = ms[ST_DENSITY]; out->ms_forces = ms[ST_FORCES]; out->ms_leapfrog = ms[ST_LEAPFROG];
+    for (int k = 0; k < ST_COUNT; ++k) out->ms_total += ms[k];
+    const DevScalars& s = *c->h_sc;
+    out->n_particles = c->N; out->n_groups = c->n_groups; out->n_neighbours = (int64_t)c->n_neigh;
+    out->nbr_min = (int32_t)s.nbr_min; out->nbr_max = (int32_t)s.nbr_max;
+    out->nbr_mean = c->N ? (double)c->n_neigh / (double)c->N : 0.0;
+    out->h_iter_max = (int32_t)s.h_iter_max; out->restarts = c->restarts_last; out->steps = c->steps;
+    out->kernel_launches = c->launches; out->dt = s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
+    return SPH_OK;
+}
+
+// ---- FP64 peak microbenchmark: 8 independent DFMA chains per thread ----
+__global__ void __launch_bounds__(256) k_dfma(double* out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == 123.456) out[0] = s;
+}
+
+int sph_measure_fp64_peak(double* tflops_out, void* cuda_stream) {
+    if (!tflops_out) return SPH_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* d = nullptr;
+    if (cudaMalloc(&d, 256) != cudaSuccess) return SPH_ERR_DEVICE;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = 148 * 8, iters = 1 << 15;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, st);
+        k_dfma<<<blocks, 256, 0, st>>>(d, iters, 0.999999, 1e-9);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return SPH_ERR_DEVICE; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double tf = 2.0 * 8.0 * (double)iters * blocks * 256 / (ms * 1e-3) * 1e-12;
+        if (rep > 0) best = std::max(best, tf);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    *tflops_out = best;
+    return SPH_OK;
+}
+
+}  // extern "C"

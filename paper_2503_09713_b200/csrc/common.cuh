@@ -1,0 +1,193 @@
+// common.cuh -- shared declarations of libsph_b200 (CUDA, sm_100a only). See include/sph_b200.h for the ABI and
+// DESIGN.md for the kernel-by-kernel design. Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <vector>
+
+#include "../../include/sph_b200.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "libsph_b200 is written for sm_100a (B200) only"
+#endif
+
+namespace sph {
+
+constexpr int kGroup = 32;          // leaf-group size bound: one warp lane per particle of a group
+constexpr double kRkern = 2.0;      // M4 support radius / h
+constexpr double kCnorm = 0.31830988618379067154;   // 1/pi
+
+// Sorted-order particle fields (SoA). Two sets are kept; the permute writes the other one.
+struct Fields {
+    double *x, *y, *z, *vx, *vy, *vz, *ax, *ay, *az, *u, *du, *h, *m;
+    uint32_t* id;
+};
+constexpr int kNumF64Fields = 13;
+
+// One record per internal radix-tree node, 64 B: tight box, max h, and the integers the traversal needs.
+// A node's index is one end of its key range (Karras convention); `other` is the other end; `split` is the
+// left child's id (right child = split + 1); a child is a leaf iff it coincides with the range end on its side.
+struct __align__(16) NodeRec {
+    double lo[3], hi[3];
+    double hmax;
+    int32_t other, split;
+};
+static_assert(sizeof(NodeRec) == 64, "NodeRec must be 64 bytes");
+
+enum Stage { ST_KEYS = 0, ST_SORT, ST_PERMUTE, ST_TREE, ST_AABB, ST_TRAVERSE, ST_SCAN, ST_DENSITY, ST_FORCES,
+             ST_LEAPFROG, ST_COUNT };
+
+enum State { S_FIELDS = 0, S_TREE = 1, S_DENSITY = 2, S_FORCES = 3 };
+
+// Device-side scalars read back by the host (one small struct, copied with one cudaMemcpyAsync).
+struct DevScalars {
+    double dt;                       // global CFL minimum (G8), stored as a double; reduced with atomicMin on bits
+    unsigned long long dt_bits;
+    unsigned int n_exceeded;         // particles that exceeded chi h^n in the last density pass
+    unsigned int n_noconv;           // particles that hit max_h_iter
+    unsigned int h_iter_max;
+    unsigned int nbr_min, nbr_max;
+    unsigned int n_groups;
+    unsigned int hmax_bits_hi;       // unused padding
+    double h_max;                    // max h^n (periodic-box check)
+    unsigned long long n_neigh;      // neighbour total (= offs[N])
+    double t;                        // simulated time (sum of the dt actually used)
+};
+
+struct TimerRec { int stage; cudaEvent_t e0, e1; };
+
+}  // namespace sph
+
+struct sph_ctx {
+    int64_t N = 0;
+    sph_box box{};
+    sph_params p{};
+    cudaStream_t stream = nullptr;
+    sph_allocator alloc{};
+    int64_t bytes_allocated = 0;
+    std::vector<void*> allocations;
+
+    sph::Fields cur{}, alt{};
+    double *rho = nullptr, *omega = nullptr, *P = nullptr, *cs = nullptr, *A = nullptr;   // A = 1/(rho^2 Omega)
+    double *nax = nullptr, *nay = nullptr, *naz = nullptr, *ndu = nullptr;                // a^{n+1}, du/dt^{n+1}
+    double* hnew = nullptr;                                                               // Newton output
+    uint64_t *key = nullptr, *key_alt = nullptr;
+    uint32_t *val = nullptr, *val_alt = nullptr;
+    // radix sort scratch
+    uint32_t* sort_hist = nullptr;      // [8][256] global digit histograms -> exclusive bases
+    uint32_t* sort_status = nullptr;    // [8][tiles][256] decoupled look-back words
+    uint32_t* sort_counters = nullptr;  // [8] dynamic tile ids
+    int64_t sort_tiles = 0;
+    // tree
+    sph::NodeRec* nodes = nullptr;      // N-1
+    int32_t* parent = nullptr;          // 2N-1
+    uint32_t* visit = nullptr;          // N-1 atomic visit flags
+    // groups
+    uint32_t* gflag = nullptr;          // N   1 at the first slot of each leaf group
+    uint32_t* gscan = nullptr;          // N+1 exclusive scan of gflag (u32)
+    uint32_t* grp_lo = nullptr;         // Ng+1 first slot of group g (grp_lo[Ng] = N)
+    int64_t n_groups = 0;
+    // neighbour cache
+    uint32_t* cnt = nullptr;            // N+1
+    uint64_t* offs = nullptr;           // N+1
+    uint32_t* nbr = nullptr;
+    uint64_t nbr_cap = 0;
+    uint64_t n_neigh = 0;
+    // scan scratch
+    uint64_t* scan_status = nullptr;
+    uint32_t* scan_counter = nullptr;
+    int64_t scan_tiles = 0;
+    // scalars
+    sph::DevScalars* d_sc = nullptr;
+    sph::DevScalars* h_sc = nullptr;    // pinned
+    double* d_dtstep = nullptr;         // dt used by predictor/corrector (device scalar)
+
+    int state = sph::S_FIELDS;
+    int restarts_last = 0;
+    int64_t steps = 0;
+    double t = 0.0;
+    int64_t launches = 0;
+    bool have_cfl_dt = false;
+
+    std::vector<sph::TimerRec> timers;
+    std::vector<cudaEvent_t> event_pool;
+    char err[512] = {0};
+};
+
+namespace sph {
+
+// ---- host-side helpers (api.cu) ----
+int fail(sph_ctx* c, int code, const char* fmt, ...);
+#define SPH_CUDA(c, call)                                                                       \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return sph::fail((c), e_ == cudaErrorMemoryAllocation ? SPH_ERR_OOM : SPH_ERR_DEVICE, \
+                             "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+#define SPH_TRY(expr)             \
+    do {                          \
+        int rc_ = (expr);         \
+        if (rc_ != SPH_OK) return rc_; \
+    } while (0)
+
+inline unsigned int div_up(int64_t a, int64_t b) { return (unsigned int)((a + b - 1) / b); }
+
+// ---- stage launchers (one per .cu file); each enqueues on c->stream and bumps c->launches ----
+int launch_keys(sph_ctx* c);                                   // keys.cu
+int launch_sort(sph_ctx* c);                                   // sort.cu   (key,val) -> sorted into key,val
+int launch_permute(sph_ctx* c);                                // permute.cu
+int launch_tree(sph_ctx* c);                                   // tree.cu   karras + groups
+int launch_aabb(sph_ctx* c);                                   // tree.cu
+int launch_traverse(sph_ctx* c, bool fill);                    // neigh.cu
+int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
+int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
+int launch_density(sph_ctx* c);                                // density.cu
+int launch_forces(sph_ctx* c);                                 // forces.cu
+int launch_predict(sph_ctx* c);                                // leapfrog.cu
+int launch_correct(sph_ctx* c);                                // leapfrog.cu
+int launch_hmax(sph_ctx* c);                                   // leapfrog.cu  max h^n -> d_sc->h_max
+int launch_adopt_acc(sph_ctx* c);                              // leapfrog.cu  a^n <- a^{n+1} (white step)
+int launch_set_dt(sph_ctx* c, double user_dt);                 // leapfrog.cu  device dt for predictor/corrector; t += dt
+int launch_scatter_orig_f64(sph_ctx* c, const double* src_sorted, double* dst_orig, int ncomp);   // permute.cu
+int launch_gather_orig_f64(sph_ctx* c, const double* src_orig, double* dst_sorted, int ncomp);    // permute.cu
+int sort_scratch_bytes(int64_t N, int64_t* tiles, size_t* status_bytes);
+int scan_scratch_tiles(int64_t N);
+
+// ---- device helpers ----
+#ifdef __CUDACC__
+__device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
+
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// M4 cubic B-spline f(q) and f'(q) (reading O6); branch-light form.
+__device__ __forceinline__ void m4(double q, double& f, double& df) {
+    double t2 = 2.0 - q;
+    double fo = 0.25 * t2 * t2 * t2;          // outer branch 1 <= q < 2
+    double dfo = -0.75 * t2 * t2;
+    double fi = 1.0 + q * q * (0.75 * q - 1.5);   // inner branch q < 1
+    double dfi = q * (2.25 * q - 3.0);
+    bool in = q < 1.0, sup = q < 2.0;
+    f = in ? fi : (sup ? fo : 0.0);
+    df = in ? dfi : (sup ? dfo : 0.0);
+}
+#endif
+
+}  // namespace sph

@@ -1,0 +1,125 @@
+// leapfrog.cu -- a7: leapfrog kick-drift-kick with a global timestep (G1-G5, order of
+// Fig. G1; u integrated like v, reading A13). Elementwise and HBM-bound. The timestep is
+// read from device memory so that a step needs no host round trip for dt (reading A14).
+#include "common.cuh"
+
+namespace sph {
+
+struct WrapBox { double lo[3], hi[3], L[3]; int periodic[3]; };
+
+__device__ __forceinline__ double wrap_pos(double r, double lo, double hi, double L, int periodic) {
+    if (periodic) {
+        if (r >= hi) r -= L;
+        else if (r < lo) r += L;
+        if (r >= hi) r = lo;       // r + L rounded up to hi
+    }
+    return r;
+}
+
+// G1-G3: v_half = v + dt/2 a; r += dt v_half (wrapped); v* = v_half + dt/2 a; same for u with du/dt
+__global__ void __launch_bounds__(256) k_predict(int64_t N, Fields f, WrapBox wb, const double* __restrict__ dtp) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double dt = *dtp, hdt = 0.5 * dt;
+    {
+        double a = f.ax[i], vh = f.vx[i] + hdt * a;
+        f.x[i] = wrap_pos(f.x[i] + dt * vh, wb.lo[0], wb.hi[0], wb.L[0], wb.periodic[0]);
+        f.vx[i] = vh + hdt * a;
+    }
+    {
+        double a = f.ay[i], vh = f.vy[i] + hdt * a;
+        f.y[i] = wrap_pos(f.y[i] + dt * vh, wb.lo[1], wb.hi[1], wb.L[1], wb.periodic[1]);
+        f.vy[i] = vh + hdt * a;
+    }
+    {
+        double a = f.az[i], vh = f.vz[i] + hdt * a;
+        f.z[i] = wrap_pos(f.z[i] + dt * vh, wb.lo[2], wb.hi[2], wb.L[2], wb.periodic[2]);
+        f.vz[i] = vh + hdt * a;
+    }
+    {
+        double d = f.du[i], uh = f.u[i] + hdt * d;
+        f.u[i] = uh + hdt * d;
+    }
+}
+
+// G5: v = v* + dt/2 (a_new - a_old); then a_old <- a_new (same for u)
+__global__ void __launch_bounds__(256) k_correct(int64_t N, Fields f, const double* __restrict__ nax,
+                                                 const double* __restrict__ nay, const double* __restrict__ naz,
+                                                 const double* __restrict__ ndu, const double* __restrict__ dtp) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double hdt = 0.5 * *dtp;
+    double a;
+    a = nax[i]; f.vx[i] = f.vx[i] + hdt * (a - f.ax[i]); f.ax[i] = a;
+    a = nay[i]; f.vy[i] = f.vy[i] + hdt * (a - f.ay[i]); f.ay[i] = a;
+    a = naz[i]; f.vz[i] = f.vz[i] + hdt * (a - f.az[i]); f.az[i] = a;
+    a = ndu[i]; f.u[i] = f.u[i] + hdt * (a - f.du[i]); f.du[i] = a;
+}
+
+// copy a^{n+1} into the a^n slots without a velocity correction (white step)
+__global__ void __launch_bounds__(256) k_adopt_acc(int64_t N, Fields f, const double* __restrict__ nax,
+                                                   const double* __restrict__ nay, const double* __restrict__ naz,
+                                                   const double* __restrict__ ndu) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    f.ax[i] = nax[i]; f.ay[i] = nay[i]; f.az[i] = naz[i]; f.du[i] = ndu[i];
+}
+
+__global__ void __launch_bounds__(256) k_hmax(int64_t N, const double* __restrict__ h, DevScalars* sc) {
+    double v = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+        v = fmax(v, h[i]);
+    v = warp_max(v);
+    if (lane_id() == 0) atomicMax((unsigned long long*)&sc->h_max, (unsigned long long)__double_as_longlong(v));
+}
+__global__ void k_hmax_reset(DevScalars* sc) { sc->h_max = 0.0; }
+
+__global__ void k_set_dt(double* dtp, DevScalars* sc, double user_dt) {
+    const double dt = (user_dt > 0.0) ? user_dt : sc->dt;
+    *dtp = dt;
+    sc->t += dt;
+}
+
+int launch_predict(sph_ctx* c) {
+    WrapBox wb;
+    for (int k = 0; k < 3; ++k) {
+        wb.lo[k] = c->box.lo[k]; wb.hi[k] = c->box.hi[k]; wb.L[k] = c->box.hi[k] - c->box.lo[k];
+        wb.periodic[k] = c->box.periodic[k];
+    }
+    k_predict<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur, wb, c->d_dtstep);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int launch_correct(sph_ctx* c) {
+    k_correct<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu, c->d_dtstep);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int launch_hmax(sph_ctx* c) {
+    k_hmax_reset<<<1, 1, 0, c->stream>>>(c->d_sc);
+    unsigned blocks = (unsigned)min((int64_t)148 * 4, (c->N + 255) / 256);
+    k_hmax<<<blocks, 256, 0, c->stream>>>(c->N, c->cur.h, c->d_sc);
+    c->launches += 2;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int launch_adopt_acc(sph_ctx* c) {
+    k_adopt_acc<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int launch_set_dt(sph_ctx* c, double user_dt) {
+    k_set_dt<<<1, 1, 0, c->stream>>>(c->d_dtstep, c->d_sc, user_dt);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+}  // namespace sph

@@ -1,0 +1,224 @@
+// sort.cu -- a2: stable LSD radix sort of (key u64, val u32), onesweep style: one upfront histogram of all
+// eight 8-bit digits, then ONE pass per digit that reads each (key,val) once and writes it once; tile prefixes
+// are resolved with a decoupled look-back over single-word (flag|count) status entries; ranking inside a tile
+// uses warp-level __match_any_sync multisplit. Replaces the paper's bitonic sort, which it
+// says dominates the tree build. HBM-bound: 8 B + 8 x 24 B = 200 B per particle.
+#include "common.cuh"
+
+namespace sph {
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kPasses = 8;
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kItems = 16;                       // keys per thread
+constexpr int kTile = kSortThreads * kItems;     // 4096 keys per tile
+constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
+
+// ---- kernel 1: histograms of all 8 digits in one read of the keys ----
+__global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ key, int64_t N,
+                                                   uint32_t* __restrict__ ghist) {
+    __shared__ uint32_t sh[kPasses][kRadix];
+    for (int i = threadIdx.x; i < kPasses * kRadix; i += blockDim.x) (&sh[0][0])[i] = 0;
+    __syncthreads();
+    const unsigned lane = lane_id();
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    int64_t n_round = (N + 31) / 32 * 32;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        bool valid = i < N;
+        unsigned act = __ballot_sync(0xffffffffu, valid);
+        if (valid) {
+            uint64_t k = key[i];
+#pragma unroll
+            for (int p = 0; p < kPasses; ++p) {
+                unsigned d = (unsigned)(k >> (p * kRadixBits)) & (kRadix - 1);
+                unsigned m = __match_any_sync(act, d);           // warp-aggregated histogram update
+                if (lane == (unsigned)(__ffs(m) - 1)) atomicAdd(&sh[p][d], __popc(m));
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kPasses * kRadix; i += blockDim.x) {
+        uint32_t v = (&sh[0][0])[i];
+        if (v) atomicAdd(&ghist[i], v);
+    }
+}
+
+// ---- kernel 2: exclusive scan of each digit histogram -> global digit bases ----
+__global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ ghist) {
+    __shared__ uint32_t wsum[kRadix / 32];
+    const unsigned d = threadIdx.x, lane = lane_id(), w = d >> 5;
+    for (int p = 0; p < kPasses; ++p) {
+        uint32_t v = ghist[p * kRadix + d], inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= (unsigned)o) inc += t;
+        }
+        if (lane == 31) wsum[w] = inc;
+        __syncthreads();
+        uint32_t base = 0;
+        for (unsigned j = 0; j < w; ++j) base += wsum[j];
+        ghist[p * kRadix + d] = base + inc - v;
+        __syncthreads();
+    }
+}
+
+// ---- kernel 3: one onesweep pass ----
+struct SortSmem {
+    uint64_t keys[kTile];
+    uint32_t vals[kTile];
+    uint32_t whist[kSortWarps][kRadix];
+    uint32_t gofs[kRadix];
+    uint32_t wsum[kRadix / 32];
+    uint32_t tile;
+};
+
+__global__ void __launch_bounds__(kSortThreads) k_onesweep(const uint64_t* __restrict__ kin,
+                                                            const uint32_t* __restrict__ vin,
+                                                            uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
+                                                            int64_t N, int shift, const uint32_t* __restrict__ gbase,
+                                                            volatile uint32_t* status, uint32_t* counter) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
+    const unsigned tid = threadIdx.x, lane = lane_id(), w = tid >> 5;
+
+    if (tid == 0) s.tile = atomicAdd(counter, 1u);   // dynamic tile id: predecessors are always already running
+    for (int i = tid; i < kSortWarps * kRadix; i += kSortThreads) (&s.whist[0][0])[i] = 0;
+    __syncthreads();
+    const uint32_t tile = s.tile;
+    const int64_t base = (int64_t)tile * kTile;
+    const int tile_n = (int)min((int64_t)kTile, N - base);
+
+    // load (warp-striped) and rank inside the warp with match_any multisplit
+    uint64_t k[kItems];
+    uint32_t rank[kItems];
+    const int64_t wbase = base + (int64_t)w * (32 * kItems) + lane;
+#pragma unroll
+    for (int i = 0; i < kItems; ++i) {
+        int64_t idx = wbase + i * 32;
+        k[i] = (idx < N) ? kin[idx] : ~0ull;
+    }
+    const unsigned lt = lanemask_lt();
+#pragma unroll
+    for (int i = 0; i < kItems; ++i) {
+        bool valid = (wbase + i * 32) < N;
+        unsigned act = __ballot_sync(0xffffffffu, valid);
+        unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
+        uint32_t prev = 0;
+        unsigned m = 0;
+        if (valid) {
+            m = __match_any_sync(act, d);
+            prev = s.whist[w][d];
+        }
+        __syncwarp();
+        if (valid && lane == (unsigned)(__ffs(m) - 1)) s.whist[w][d] = prev + __popc(m);
+        __syncwarp();
+        rank[i] = prev + __popc(m & lt);
+    }
+    __syncthreads();
+
+    // per digit (thread d): exclusive scan over the warps, tile count, look-back, tile-local digit start
+    {
+        const unsigned d = tid;
+        uint32_t run = 0;
+#pragma unroll
+        for (int ww = 0; ww < kSortWarps; ++ww) {
+            uint32_t t = s.whist[ww][d];
+            s.whist[ww][d] = run;
+            run += t;
+        }
+        volatile uint32_t* my = status + (size_t)tile * kRadix + d;
+        *my = (tile == 0 ? kFlagIncl : kFlagAgg) | run;
+        // tile-local exclusive scan of the 256 digit counts
+        uint32_t inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= (unsigned)o) inc += t;
+        }
+        if (lane == 31) s.wsum[w] = inc;
+        __syncthreads();
+        uint32_t dstart = inc - run;
+        for (unsigned j = 0; j < w; ++j) dstart += s.wsum[j];
+        // decoupled look-back
+        uint32_t excl = 0;
+        if (tile > 0) {
+            int64_t t = (int64_t)tile - 1;
+            for (;;) {
+                uint32_t v = status[(size_t)t * kRadix + d];
+                uint32_t flag = v & ~kValMask;
+                if (flag == 0) continue;              // predecessor has not published yet: spin
+                excl += v & kValMask;
+                if (flag == kFlagIncl) break;
+                --t;
+            }
+            *my = kFlagIncl | (excl + run);
+        }
+        s.gofs[d] = gbase[d] + excl - dstart;
+#pragma unroll
+        for (int ww = 0; ww < kSortWarps; ++ww) s.whist[ww][d] += dstart;
+    }
+    __syncthreads();
+
+    // scatter into shared memory in tile-sorted order
+#pragma unroll
+    for (int i = 0; i < kItems; ++i) {
+        int64_t idx = wbase + i * 32;
+        if (idx < N) {
+            unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
+            uint32_t slot = s.whist[w][d] + rank[i];
+            s.keys[slot] = k[i];
+            s.vals[slot] = vin[idx];
+        }
+    }
+    __syncthreads();
+
+    // coalesced runs out to global memory
+    for (int j = tid; j < tile_n; j += kSortThreads) {
+        uint64_t kk = s.keys[j];
+        unsigned d = (unsigned)(kk >> shift) & (kRadix - 1);
+        uint32_t pos = s.gofs[d] + (uint32_t)j;
+        kout[pos] = kk;
+        vout[pos] = s.vals[j];
+    }
+}
+
+int sort_scratch_bytes(int64_t N, int64_t* tiles, size_t* status_bytes) {
+    *tiles = (N + kTile - 1) / kTile;
+    *status_bytes = (size_t)kPasses * (size_t)(*tiles) * kRadix * sizeof(uint32_t);
+    return SPH_OK;
+}
+
+int launch_sort(sph_ctx* c) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPH_CUDA(c, cudaFuncSetAttribute(k_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
+        attr_set = true;
+    }
+    const int64_t N = c->N, tiles = c->sort_tiles;
+    const size_t status_per_pass = (size_t)tiles * kRadix;
+    SPH_CUDA(c, cudaMemsetAsync(c->sort_hist, 0, kPasses * kRadix * sizeof(uint32_t), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(c->sort_status, 0, kPasses * status_per_pass * sizeof(uint32_t), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(c->sort_counters, 0, kPasses * sizeof(uint32_t), c->stream));
+    unsigned hb = (unsigned)min((int64_t)148 * 8, (N + 255) / 256);
+    k_sort_hist<<<hb, 256, 0, c->stream>>>(c->key, N, c->sort_hist);
+    k_sort_bases<<<1, kRadix, 0, c->stream>>>(c->sort_hist);
+    c->launches += 2;
+    uint64_t *kin = c->key, *kout = c->key_alt;
+    uint32_t *vin = c->val, *vout = c->val_alt;
+    for (int p = 0; p < kPasses; ++p) {
+        k_onesweep<<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
+            kin, vin, kout, vout, N, p * kRadixBits, c->sort_hist + p * kRadix,
+            c->sort_status + p * status_per_pass, c->sort_counters + p);
+        c->launches++;
+        uint64_t* tk = kin; kin = kout; kout = tk;
+        uint32_t* tv = vin; vin = vout; vout = tv;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    // kPasses is even: the result is back in c->key / c->val
+    return SPH_OK;
+}
+
+}  // namespace sph
