@@ -1,0 +1,266 @@
+#!/usr/bin/env python
+"""bench.py -- SPH particle-updates/s per full leapfrog step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cube256|cube128|sod|disc|...] [--impl reference]
+
+A "step" is one pass of the whole hot path: predictor, Morton keys, onesweep sort,
+permute, Karras tree, AABB/hmax, traversal -> neighbour cache, h/density Newton iteration, forces + CFL dt,
+corrector. Default workload: BASELINE.json configs[2], the 256^3 uniform periodic cube the metric's target is
+quoted on (16.8 M particles, ~13 GB resident: far larger than L2, so no L2 flush is needed between steps).
+Multi-GPU: replicas only (the path has no exchange step in scope) -- every rank runs the same
+workload with a different seed; value = particles stepped by all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "sph_particle_updates_per_sec_per_full_step"
+UNIT = "particle-updates/s"
+
+# Algorithmic work per unit, stated in DESIGN.md "Rooflines": FP64 flop per neighbour pair (fma = 2, div = sqrt = 1)
+FLOP_PER_PAIR_DENSITY_GATHER = 11     # separation, d^2, sqrt (once per pair per density solve)
+FLOP_PER_PAIR_DENSITY_SWEEP = 16      # q, f, f', two accumulations (per pair per Newton sweep)
+FLOP_PER_PAIR_FORCE = 93              # Eq. 3-6, 8-10 per pair
+FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair (count + fill = 2 tests)
+
+
+def make_workload(name: str, seed_offset: int = 0):
+    from paper_2503_09713_b200 import workloads as W
+    seed = W.DEFAULT_SEED + seed_offset
+    if name.startswith("cube"):
+        n = int(name[4:])
+        return W.cube(n, jitter=0.1, seed=seed, steps=5, name=f"C2-recipe uniform periodic cube {n}^3")
+    if name == "sod":
+        return W.config(1)
+    if name.startswith("disc"):
+        n = int(name[4:] or 10_000_000)
+        return W.disc(n, seed=seed)
+    if name == "c0":
+        return W.config(0)
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 3 + k and r[3 + k].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(self.rows[0][1]) if self.rows[0][1].replace(".", "").isdigit() else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(self.rows), "reasons": reasons}
+
+
+def oracle_step_rate(n_side: int, steps: int, warmup: int):
+    """Time the oracle (as it stands, 1 thread) on the C2 recipe at n_side^3 particles."""
+    import oracle as O
+    from paper_2503_09713_b200 import workloads as W
+    w = W.cube(n_side, jitter=0.1, steps=steps)
+    t_init = time.perf_counter()
+    s = O.State(w, "grid")
+    t_init = time.perf_counter() - t_init
+    for _ in range(warmup):
+        s.step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        s.step()
+    dt = time.perf_counter() - t0
+    return w.n * steps / dt, dt / steps, w.n, t_init
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (reference arm for this tier)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_side = 40
+    rate, s_per_step, n, _ = oracle_step_rate(n_side, args.steps, args.warmup)
+    sample = f"C2 recipe at {n_side}^3 = {n} particles (bounded sample of the 256^3 workload), {args.steps} full oracle steps"
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": make_workload(args.workload).name if False else f"{args.workload} (oracle sample {n_side}^3)",
+                       "n_particles": n, "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cube256")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2503_09713_b200 import binding as B, build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not os.path.exists(B.LIB_PATH):
+        if rank == 0:
+            build.build()
+        if world > 1:
+            dist.barrier()
+
+    w = make_workload(args.workload, seed_offset=rank)
+    n = w.n
+    sim = B.Sim.from_workload(w)          # inputs resident in HBM; includes the white step
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        sim.step_leapfrog()
+    barrier()
+    sim.reset_timers()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        sim.step_leapfrog()
+    e1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    ms = e0.elapsed_time(e1)
+    st = sim.stats()
+    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    ntot = torch.tensor([float(n)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ntot, op=dist.ReduceOp.SUM)
+    ms_all, n_all = float(tmax.item()), float(ntot.item())
+    value = n_all * args.steps / (ms_all * 1e-3)
+
+    # ---- end-to-end through the C ABI with HOST buffers: upload state, step, download results, every step
+    e2e = None
+    if not args.no_e2e:
+        host = sim.get_fields(("pos", "vel", "u", "h", "acc", "dudt"), host=True)
+        out = {k: torch.empty_like(v).pin_memory() for k, v in
+               sim.get_fields(("pos", "vel", "u", "h", "rho", "acc", "dudt"), host=True).items()}
+        h2d = sum(v.numel() * 8 for v in host.values())
+        d2h = sum(v.numel() * 8 for v in out.values())
+        k_e2e = max(2, min(args.steps, 3))
+        for it in range(1 + k_e2e):
+            if it == 1:
+                barrier()
+                t0 = time.perf_counter()
+            sim.set_fields(**host)
+            sim.step_leapfrog()
+            res = sim.get_fields(tuple(out.keys()), host=True, out=out)
+            for k in host:
+                host[k].copy_(res[k])
+        barrier()
+        t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        e2e = {"value": n_all * k_e2e / float(t_e2e.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": k_e2e}
+
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+        hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"
+        fp64_peak = B.measure_fp64_peak()      # TFLOP/s, DFMA microbenchmark run now on this GPU
+        K = args.steps
+        pairs = st["n_neighbours"]             # pairs in the cache of the last step (self included)
+        sweeps = max(st["h_iter_max"], 1) + 1  # upper bound on Newton sweeps + the Omega pass
+        per_stage = {k[3:]: st[k] / K for k in st if k.startswith("ms_") and k != "ms_total"}
+        flops = {"density": pairs * (FLOP_PER_PAIR_DENSITY_GATHER + FLOP_PER_PAIR_DENSITY_SWEEP * sweeps),
+                 "forces": pairs * FLOP_PER_PAIR_FORCE,
+                 "traverse": pairs * FLOP_PER_PAIR_TEST * 2}
+        bytes_ = {"keys": 36 * n, "sort": 200 * n, "permute": 216 * n, "tree": 60 * n, "aabb": 148 * n,
+                  "scan": 12 * n, "leapfrog": 272 * n}
+        kernels = {}
+        for k, v in per_stage.items():
+            if k in flops:
+                ach = flops[k] / (v * 1e-3) * 1e-12
+                kernels[k] = {"ms": v, "bound": "alu", "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s (fp64)", "frac": ach / fp64_peak}
+            else:
+                ach = bytes_[k] / (v * 1e-3) * 1e-9 if v > 0 else 0.0
+                kernels[k] = {"ms": v, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
+        dom = max(per_stage, key=per_stage.get)
+        roofline = dict(kernels[dom])
+        roofline.update({"kernel": dom, "traffic": None,
+                         "peak_source": "sph_measure_fp64_peak DFMA microbenchmark, this run" if dom in flops else hbm_src,
+                         "share_of_step": per_stage[dom] / sum(per_stage.values())})
+        cpu = None
+        if not args.no_cpu_baseline:
+            rate, s_per_step, n_s, t_init = oracle_step_rate(40, 1, 0)
+            cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"C2 recipe at 40^3 = {n_s} particles, 1 full oracle leapfrog step ({s_per_step:.1f} s) after its white step ({t_init:.1f} s)"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": "M4",
+                           "hfact": w.hfact, "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "l2": "inputs (~0.8 kB/particle resident) larger than the 126 MB L2; no flush",
+                           "restarts_last_step": st["restarts"], "h_iter_max": st["h_iter_max"]},
+                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(st["kernel_launches"]),
+                "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
+                "context": {"paper_a100_particles_per_s": 12e6, "fp64_peak_tflops_measured": fp64_peak,
+                            "hbm_peak_gbs": hbm_peak, "bytes_allocated": st["bytes_allocated"]}}
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

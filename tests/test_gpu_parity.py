@@ -1,0 +1,276 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): Morton keys, sort permutation, tree tables, node boxes and neighbour sets
+bit-exact; rho and h within 1e-10 relative; accelerations and du/dt within 1e-8 of the global max.
+Protocol P1: the oracle is always evaluated on the state the GPU stage started from.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_2503_09713_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHO_H = 1e-10      # relative, per particle (north_star)
+TOL_ACC = 1e-8         # of the global max |a| (or max |du/dt|) (north_star)
+BAND = 2e-12           # pairs with |d^2/rc^2 - 1| < BAND are listed and excluded (north_star: 1e-12 of r = 2h)
+
+
+def _sim(w, **kw):
+    from paper_2503_09713_b200 import binding as B
+    return B.Sim.from_workload(w, **kw)
+
+
+def _np(fields):
+    return {k: v.cpu().numpy() for k, v in fields.items()}
+
+
+def _near_cutoff_pairs(pos, h, box, chi, offs, idx):
+    """Pairs of a CSR cache whose d^2 is within BAND of the cutoff (either side would be tolerated)."""
+    L = np.array([box.hi[k] - box.lo[k] for k in range(3)])
+    a = np.repeat(np.arange(offs.size - 1), np.diff(offs).astype(np.int64))
+    d = pos[:, a] - pos[:, idx]
+    for k in range(3):
+        if box.periodic[k]:
+            d[k] = np.where(d[k] > 0.5 * L[k], d[k] - L[k], np.where(d[k] < -0.5 * L[k], d[k] + L[k], d[k]))
+    d2 = (d * d).sum(axis=0)
+    rc2 = (2.0 * chi * np.maximum(h[a], h[idx])) ** 2
+    return int((np.abs(d2 / rc2 - 1.0) < BAND).sum())
+
+
+def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None):
+    """Compare every stage of one evaluation. `state` = (pos, vel, u) in original order the evaluation started
+    from (default: the workload's initial conditions); hn = the h^n it started from."""
+    box, p = O.workload_box_params(w)
+    pos, vel, u = state if state is not None else (w.pos, w.vel, w.u)
+    hn = w.h0 if hn is None else hn
+    n = w.n
+    # a1, a2: keys and permutation
+    skey, perm = O.sort_keys(O.morton_keys(pos, box))
+    gkey, gperm = sim.get_keys_perm()
+    assert np.array_equal(gkey, skey), "sorted Morton keys differ"
+    if np.unique(skey).size == n:
+        assert np.array_equal(gperm, perm), "sort permutation differs"
+    else:   # equal keys: ties follow the slot order at sort time, which is the original order only at step 0
+        assert np.array_equal(np.sort(gperm), np.arange(n)) and np.array_equal(O.morton_keys(pos, box)[gperm], skey)
+        if state is None:
+            assert np.array_equal(gperm, perm)
+    # a3: tree tables (Table B2 conventions)
+    t = O.tree(skey)
+    g = sim.get_tree()
+    for k in ("left", "right", "lflag", "rflag", "parent", "rlo", "rhi"):
+        assert np.array_equal(g[k], t[k]), f"tree table {k} differs"
+    # oracle physics on the same state
+    ev = O.evaluate(pos, vel, w.mass, u, hn, box, p, "grid")
+    st = sim.stats()
+    if expect_restarts is not None:
+        assert ev["restarts"] == expect_restarts
+    assert st["restarts"] == ev["restarts"], "chi-restart counts differ"
+    f = _np(sim.get_fields())
+    # a3b: node boxes / hmax are those of the LAST cache build, i.e. with h^n of the final pass. After r restarts
+    # h^n of the final pass is unknown to the test unless r == 0; check boxes always, hmax when r == 0.
+    ps = pos[:, gperm]
+    box6, hmax = O.aabb(t, ps, hn[gperm])
+    assert np.array_equal(g["aabb"], box6), "node boxes differ"
+    if ev["restarts"] == 0:
+        assert np.array_equal(g["hmax"], hmax), "node hmax differs"
+        # a4: neighbour sets (sorted-slot indices), compared as sets per particle
+        oo, oi = O.neighbours(ps, hn[gperm], box, p.chi, "grid")
+        go, gi = sim.get_neighbours()
+        assert _near_cutoff_pairs(ps, hn[gperm], box, p.chi, oo, oi) == 0   # nothing to exclude on these inputs
+        assert np.array_equal(go, oo), "neighbour counts differ"
+        order = np.lexsort((gi, np.repeat(np.arange(n), np.diff(go).astype(np.int64))))
+        assert np.array_equal(gi[order], oi), "neighbour sets differ"
+    assert st["n_neighbours"] == ev["n_neigh"]
+    # a5: h, rho (1e-10 relative), Omega
+    assert np.max(np.abs(f["h"] / ev["h"] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["rho"] / ev["rho"] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["omega"] - ev["omega"])) < 1e-9
+    # a6: forces, du/dt (1e-8 of the global max), dt
+    # (floored by the natural scales c_s^2/h and c_s^3/h so that an exactly balanced lattice, where a = 0 up to
+    # round-off, is not compared against its own rounding noise)
+    cs2 = p.gamma * (p.gamma - 1.0) * np.abs(u).max() if p.eos == 0 else p.cs0 ** 2
+    amax = max(np.abs(ev["acc"]).max(), 1e-3 * cs2 / ev["h"].max())
+    dmax = max(np.abs(ev["dudt"]).max(), 1e-3 * cs2 ** 1.5 / ev["h"].max())
+    assert np.max(np.abs(f["acc"] - ev["acc"])) <= TOL_ACC * amax
+    assert np.max(np.abs(f["dudt"] - ev["dudt"])) <= TOL_ACC * dmax
+    assert st["dt"] == pytest.approx(ev["dt"], rel=1e-12)
+    return ev, f
+
+
+def test_c0_stage_parity():
+    """BASELINE config 0: 16^3 jittered periodic cube, one build + density + force."""
+    w = W.config(0)
+    sim = _sim(w)
+    ev, f = _stage_parity(w, sim, expect_restarts=0)
+    st = sim.stats()
+    assert st["n_groups"] == w.n // 32 and st["nbr_min"] >= 60
+    assert np.all(np.abs((w.mass * f["acc"]).sum(axis=1)) < 1e-13 * np.abs(f["acc"]).max())   # sum m a = 0
+    sim.close()
+
+
+@pytest.mark.parametrize("make", [
+    lambda: W.random_cloud(5000, seed=3),                      # clustered, periodic, chi-restarts at init
+    lambda: W.random_cloud(3777, seed=5, periodic=False),      # open boundaries, ragged tail (3777 = 118*32 + 1)
+    lambda: W.sod(16, 12),                                     # density jump, non-cubic box (cube embedding of keys)
+    lambda: W.cube(12, jitter=0.0, vel_amp=0.0),               # exact lattice: many equidistant pairs
+    lambda: W.disc(6000, seed=2),                              # isothermal EOS + point mass + strongly varying h
+], ids=["cloud_periodic", "cloud_open_ragged", "sod_small", "lattice", "disc_small"])
+def test_stage_parity_small(make):
+    w = make()
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    sim.close()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 32, 33, 64, 65, 4097])
+def test_edge_sizes(n):
+    """Degenerate and ragged sizes: single particle, a single group, one particle past a tile/group boundary."""
+    rng = np.random.default_rng(n)
+    w = W.random_cloud(max(n, 40), seed=n, periodic=False, clustered=False)
+    sel = np.arange(n)
+    w.pos, w.vel, w.mass, w.u = (np.ascontiguousarray(w.pos[:, sel]), np.ascontiguousarray(w.vel[:, sel]),
+                                 w.mass[sel].copy(), w.u[sel].copy())
+    w.h0 = np.full(n, 0.9 * (1.0 / max(n, 8)) ** (1 / 3))
+    if n < 8:   # too few particles for the h equation to have a root: check build_tree only (keys, tree, cache)
+        from paper_2503_09713_b200 import binding as B
+        sim = B.Sim.from_workload(w, white_step=False)
+        sim.build_tree()
+        box, p = O.workload_box_params(w)
+        skey, perm = O.sort_keys(O.morton_keys(w.pos, box))
+        gk, gp = sim.get_keys_perm()
+        assert np.array_equal(gk, skey) and np.array_equal(gp, perm)
+        t, g = O.tree(skey), sim.get_tree()
+        for k in ("left", "right", "lflag", "rflag", "parent", "rlo", "rhi"):
+            assert np.array_equal(g[k], t[k])
+        oo, oi = O.neighbours(w.pos[:, perm], w.h0[perm], box, p.chi, "brute")
+        go, gi = sim.get_neighbours()
+        assert np.array_equal(go, oo) and np.array_equal(np.sort(gi), np.sort(oi))
+        sim.close()
+        return
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    sim.close()
+
+
+def test_duplicate_keys_and_coincident_particles():
+    """Equal Morton keys (tie-break on the sorted index, reading O3) and exactly coincident positions."""
+    w = W.random_cloud(600, seed=9, periodic=True, clustered=False)
+    w.pos[:, 100:104] = w.pos[:, 100:101]                 # four coincident particles
+    w.pos[:, 200] = w.pos[:, 201] + 1e-9                  # same key cell, different position
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    sim.close()
+
+
+def test_multi_step_trajectory_and_stage_parity():
+    """Protocol P1 + P2 on a C0-like input: 5 leapfrog steps; stage parity before every step on the GPU's own
+    state, trajectory parity against the oracle's own run, conservation checks."""
+    w = W.cube(16, jitter=0.05, vel_amp=0.02, seed=7)
+    sim = _sim(w)
+    s = O.State(w, "grid")
+    f0 = _np(sim.get_fields())
+    e0 = (w.mass * (0.5 * (f0["vel"] ** 2).sum(axis=0) + f0["u"])).sum()
+    for step in range(5):
+        before = _np(sim.get_fields(("pos", "vel", "u", "h", "acc", "dudt")))
+        dt_gpu = sim.step_leapfrog(want_dt=True)
+        dt_or = s.step()
+        assert dt_gpu == pytest.approx(dt_or, rel=1e-9)
+        # P1: redo this step's evaluation in the oracle from the GPU's pre-step state
+        box, p = O.workload_box_params(w)
+        st = O.State.__new__(O.State)
+        st.box, st.p, st.mode = box, p, "grid"
+        st.pos, st.vel, st.m, st.u, st.h = (before["pos"].copy(), before["vel"].copy(), w.mass.copy(),
+                                            before["u"].copy(), before["h"].copy())
+        st.acc, st.dudt, st.rho, st.omega = before["acc"].copy(), before["dudt"].copy(), np.empty(w.n), np.empty(w.n)
+        st.t, st.dt = 0.0, dt_gpu
+        st.step(dt_gpu)
+        after = _np(sim.get_fields())
+        assert np.max(np.abs(after["pos"] - st.pos)) < 1e-14
+        assert np.max(np.abs(after["h"] / st.h - 1)) < TOL_RHO_H
+        assert np.max(np.abs(after["rho"] / st.rho - 1)) < TOL_RHO_H
+        assert np.max(np.abs(after["acc"] - st.acc)) <= TOL_ACC * np.abs(st.acc).max()
+        assert np.max(np.abs(after["dudt"] - st.dudt)) <= TOL_ACC * np.abs(st.dudt).max()
+        assert np.max(np.abs(after["vel"] - st.vel)) < 1e-12 * max(np.abs(st.vel).max(), 1.0)
+    # P2: trajectory parity against the oracle's own 5-step run (round-off grows; documented tolerance 1e-9)
+    after = _np(sim.get_fields())
+    assert np.max(np.abs(after["pos"] - s.pos)) < 1e-9
+    assert np.max(np.abs(after["vel"] - s.vel)) < 1e-9
+    assert np.max(np.abs(after["u"] - s.u)) < 1e-9
+    e1 = (w.mass * (0.5 * (after["vel"] ** 2).sum(axis=0) + after["u"])).sum()
+    assert abs(e1 / e0 - 1) < 1e-5
+    assert np.all(np.abs((w.mass * after["vel"]).sum(axis=1) - (w.mass * f0["vel"]).sum(axis=1)) < 1e-14)
+    assert sim.stats()["steps"] == 5
+    sim.close()
+
+
+def test_host_buffers_and_set_fields_roundtrip():
+    """The e2e path of bench.py: host buffers in, step, host buffers out; equals the device-buffer path."""
+    import torch
+    w = W.cube(16, jitter=0.05, vel_amp=0.02, seed=3)
+    a = _sim(w)                                   # device inputs
+    b = _sim(w, device_inputs=False)              # host (numpy) inputs
+    fa = _np(a.get_fields())
+    fb = {k: v.numpy() for k, v in b.get_fields(host=True).items()}
+    for k in fa:
+        assert np.array_equal(fa[k], fb[k]), k
+    # upload the state through host buffers, step, and compare with the resident path
+    b.set_fields(pos=fb["pos"], vel=fb["vel"], u=fb["u"], h=fb["h"], acc=fb["acc"], dudt=fb["dudt"])
+    a.step_leapfrog()
+    b.step_leapfrog()
+    fa = _np(a.get_fields())
+    fb = {k: v.numpy() for k, v in b.get_fields(host=True).items()}
+    for k in ("pos", "vel", "u", "h", "rho"):
+        assert np.allclose(fa[k], fb[k], rtol=1e-12, atol=1e-15), k
+    a.close()
+    b.close()
+
+
+def test_error_paths():
+    from paper_2503_09713_b200 import binding as B
+    w = W.cube(8, jitter=0.0, vel_amp=0.0)
+    w.h0 = np.full(w.n, 0.2)                      # 2 * 2 * 1.1 * 0.2 = 0.88 < 1 passes; 0.3 must fail
+    sim = B.Sim.from_workload(w, white_step=False)
+    with pytest.raises(B.SphError) as e:
+        sim.compute_density()
+    assert e.value.code == -7                     # SPH_ERR_ORDER
+    with pytest.raises(B.SphError) as e:
+        sim.step_leapfrog()
+    assert e.value.code == -7
+    sim.close()
+    w.h0 = np.full(w.n, 0.3)
+    with pytest.raises(B.SphError) as e:
+        B.Sim.from_workload(w)
+    assert e.value.code == -6                     # SPH_ERR_PERIODIC_TOO_SMALL
+
+
+@pytest.mark.parametrize("make", [
+    lambda: W.random_cloud(5000, seed=3),
+    lambda: W.random_cloud(4000, seed=8, periodic=False),
+    lambda: W.disc(8000, seed=4),
+    lambda: W.cube(20, jitter=0.3, vel_amp=0.0, seed=2),
+], ids=["cloud_periodic", "cloud_open", "disc", "cube_jitter"])
+def test_neighbour_cache_build_only(make):
+    """a1-a4 alone (sph_build_tree without the h iteration): sets for the given h^n = h0, bit-exact, on inputs
+    with strongly varying h (lists up to several hundred entries, multi-level traversal)."""
+    from paper_2503_09713_b200 import binding as B
+    w = make()
+    sim = B.Sim.from_workload(w, white_step=False)
+    sim.build_tree()
+    box, p = O.workload_box_params(w)
+    _, gperm = sim.get_keys_perm()
+    ps, hs = w.pos[:, gperm], w.h0[gperm]
+    oo, oi = O.neighbours(ps, hs, box, p.chi, "grid")
+    go, gi = sim.get_neighbours()
+    assert _near_cutoff_pairs(ps, hs, box, p.chi, oo, oi) == 0
+    assert np.array_equal(go, oo)
+    order = np.lexsort((gi, np.repeat(np.arange(w.n), np.diff(go).astype(np.int64))))
+    assert np.array_equal(gi[order], oi)
+    g = sim.get_tree()
+    t = O.tree(O.sort_keys(O.morton_keys(w.pos, box))[0])
+    box6, hmax = O.aabb(t, ps, hs)
+    assert np.array_equal(g["aabb"], box6) and np.array_equal(g["hmax"], hmax)
+    st = sim.stats()
+    assert st["nbr_min"] == np.diff(oo).min() and st["nbr_max"] == np.diff(oo).max()
+    sim.close()
