@@ -159,6 +159,7 @@ def test_duplicate_keys_and_coincident_particles():
     w = W.random_cloud(600, seed=9, periodic=True, clustered=False)
     w.pos[:, 100:104] = w.pos[:, 100:101]                 # four coincident particles
     w.pos[:, 200] = w.pos[:, 201] + 1e-9                  # same key cell, different position
+    w.h0 = np.minimum(w.h0, 0.2)                          # minimum image needs 2 R_kern chi h_max < L = 1
     sim = _sim(w)
     _stage_parity(w, sim)
     sim.close()
