@@ -106,35 +106,53 @@ __global__ void k_h0_fallback(int64_t N, const double* __restrict__ m, const dou
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) h[i] = hfact * cbrt(m[i] * vol / *mtot);
 }
-__global__ void k_store_total(const uint64_t* offs, int64_t N, DevScalars* sc) { sc->n_neigh = offs[N]; }
 
-// neighbour cache for the current tree and h^n: hmax -> AABB -> count -> scan -> (sync) -> fill
+// (re)allocate one pool of the neighbour cache
+template <typename T>
+static int grow_pool(sph_ctx* c, T** pool, uint64_t* cap, uint64_t want) {
+    if (*pool) dfree(c, *pool);
+    *pool = nullptr;
+    *cap = 0;
+    SPH_TRY(dalloc(c, pool, (size_t)want));
+    *cap = want;
+    return SPH_OK;
+}
+
+// neighbour cache for the current tree and h^n: hmax -> AABB -> single traversal pass (count, allocate, fill per
+// group from bump allocators). The pass is repeated with larger pools if one of them overflowed (first build,
+// or a cache that grew by more than the slack since the previous step).
 static int cache_build(sph_ctx* c) {
     { StageTimer t(c, ST_AABB); SPH_TRY(launch_hmax(c)); SPH_TRY(launch_aabb(c)); }
-    { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c, false)); }
-    {
-        StageTimer t(c, ST_SCAN);
-        SPH_TRY(launch_scan_u32_u64(c, c->cnt, c->offs, c->N, nullptr));
-        k_store_total<<<1, 1, 0, c->stream>>>(c->offs, c->N, c->d_sc);
-        c->launches++;
+    for (int attempt = 0;; ++attempt) {
+        { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c)); }
+        SPH_TRY(read_scalars(c));
+        const DevScalars& s = *c->h_sc;
+        for (int k = 0; k < 3; ++k)
+            if (c->box.periodic[k] && !(2.0 * kRkern * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
+                return fail(c, SPH_ERR_PERIODIC_TOO_SMALL, "periodic axis %d: 2 R_kern chi h_max = %g >= L = %g", k,
+                            2.0 * kRkern * c->p.chi * s.h_max, c->box.hi[k] - c->box.lo[k]);
+        if (s.n_cand_overflow)
+            return fail(c, SPH_ERR_CAP, "%u leaf groups have more than 65535 candidates (16-bit local index)",
+                        s.n_cand_overflow);
+        c->n_groups = s.n_groups;
+        c->nc_max = s.nc_max;
+        c->n_neigh = s.n_neigh;
+        bool redo = false;
+        if (s.list_cursor > c->list_cap) {
+            SPH_TRY(grow_pool(c, &c->lists, &c->list_cap, s.list_cursor + s.list_cursor / 8 + 4096));
+            redo = true;
+        }
+        if (s.bkt_cursor > c->bkt_cap) {
+            SPH_TRY(grow_pool(c, &c->bkt, &c->bkt_cap, s.bkt_cursor + s.bkt_cursor / 8 + 1024));
+            redo = true;
+        }
+        if ((uint64_t)s.n_groups > c->ginfo_cap) {
+            SPH_TRY(grow_pool(c, &c->ginfo, &c->ginfo_cap, (uint64_t)s.n_groups + s.n_groups / 8 + 64));
+            redo = true;
+        }
+        if (!redo) break;
+        if (attempt >= 2) return fail(c, SPH_ERR_DEVICE, "neighbour cache pools did not converge");
     }
-    SPH_TRY(read_scalars(c));
-    const DevScalars& s = *c->h_sc;
-    for (int k = 0; k < 3; ++k)
-        if (c->box.periodic[k] && !(2.0 * kRkern * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
-            return fail(c, SPH_ERR_PERIODIC_TOO_SMALL, "periodic axis %d: 2 R_kern chi h_max = %g >= L = %g", k,
-                        2.0 * kRkern * c->p.chi * s.h_max, c->box.hi[k] - c->box.lo[k]);
-    c->n_neigh = s.n_neigh;
-    c->n_groups = s.n_groups;
-    if (c->n_neigh > c->nbr_cap) {
-        dfree(c, c->nbr);
-        c->nbr = nullptr;
-        c->nbr_cap = 0;
-        uint64_t cap = c->n_neigh + c->n_neigh / 8 + 1024;
-        SPH_TRY(dalloc(c, &c->nbr, (size_t)cap));
-        c->nbr_cap = cap;
-    }
-    { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c, true)); }
     return SPH_OK;
 }
 
@@ -211,7 +229,8 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->parent, 2 * n));
     SPH_TRY(dalloc(c, &c->visit, n));
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
-    SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->offs, n + 1));
+    SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
+    // cache pools start empty: the first traversal only counts, then they are sized from its totals
     c->scan_tiles = scan_scratch_tiles(N);
     SPH_TRY(dalloc(c, &c->scan_status, (size_t)c->scan_tiles));
     SPH_TRY(dalloc(c, &c->scan_counter, 4));
@@ -452,11 +471,20 @@ int sph_get_tree(sph_ctx* c, sph_mem mem, int32_t* left, int32_t* right, uint8_t
 int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
     SPH_TRY(check_ctx(c));
     if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no neighbour cache built");
+    // the cache is group-local (bucket tables + 16-bit lists); convert to a CSR over sorted slots on request
+    SPH_TRY(launch_scan_u32_u64(c, c->cnt, c->offs, c->N, nullptr));
     SPH_TRY(copy_raw(c, mem, offs, c->offs, (size_t)(c->N + 1) * sizeof(uint64_t)));
     if (idx) {
         if (cap < c->n_neigh) return fail(c, SPH_ERR_CAP, "idx capacity %llu < %llu neighbours", (unsigned long long)cap,
                                           (unsigned long long)c->n_neigh);
-        SPH_TRY(copy_raw(c, mem, idx, c->nbr, (size_t)c->n_neigh * sizeof(uint32_t)));
+        uint32_t* tmp = nullptr;
+        uint32_t* dst = idx;
+        if (mem == SPH_MEM_HOST) { SPH_TRY(dalloc(c, &tmp, (size_t)c->n_neigh + 1)); dst = tmp; }
+        int rc = launch_cache_to_csr(c, dst);
+        if (rc == SPH_OK && tmp) rc = copy_raw(c, mem, idx, tmp, (size_t)c->n_neigh * sizeof(uint32_t));
+        cudaStreamSynchronize(c->stream);
+        if (tmp) dfree(c, tmp);
+        if (rc != SPH_OK) return rc;
     }
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     return SPH_OK;

@@ -36,6 +36,11 @@ struct __align__(16) NodeRec {
 };
 static_assert(sizeof(NodeRec) == 64, "NodeRec must be 64 bytes");
 
+// One bucket of a group's candidate array: sorted slots [lo, lo + n) hold local candidates [cstart, cstart + n),
+// n = next entry's cstart - cstart (the table ends with a sentinel whose cstart is the group's candidate count).
+struct BucketRec { uint32_t lo, cstart; };
+struct __align__(16) GroupRec { uint32_t bkt_off_lo, bkt_off_hi, nb, nc; };
+
 enum Stage { ST_KEYS = 0, ST_SORT, ST_PERMUTE, ST_TREE, ST_AABB, ST_TRAVERSE, ST_SCAN, ST_DENSITY, ST_FORCES,
              ST_LEAPFROG, ST_COUNT };
 
@@ -54,6 +59,13 @@ struct DevScalars {
     double h_max;                    // max h^n (periodic-box check)
     unsigned long long n_neigh;      // neighbour total (= offs[N])
     double t;                        // simulated time (sum of the dt actually used)
+    // neighbour-cache allocation state of the last traversal (bump allocators + limits seen)
+    unsigned long long list_cursor;  // 16-bit list entries handed out (each group's block padded to 8 entries)
+    unsigned long long bkt_cursor;   // bucket-table entries handed out (nb + 1 per group)
+    unsigned int nc_max;             // largest candidate count of any group
+    unsigned int nb_max;             // largest bucket count of any group
+    unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
+    unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
 };
 
 struct TimerRec { int stage; cudaEvent_t e0, e1; };
@@ -89,11 +101,18 @@ struct sph_ctx {
     uint32_t* gscan = nullptr;          // N+1 exclusive scan of gflag (u32)
     uint32_t* grp_lo = nullptr;         // Ng+1 first slot of group g (grp_lo[Ng] = N)
     int64_t n_groups = 0;
-    // neighbour cache
-    uint32_t* cnt = nullptr;            // N+1
-    uint64_t* offs = nullptr;           // N+1
-    uint32_t* nbr = nullptr;
-    uint64_t nbr_cap = 0;
+    // neighbour cache, group-local (a4): per group a bucket table (slot ranges = the group's
+    // candidate array) and per particle an ascending list of 16-bit indices into that candidate array
+    uint32_t* cnt = nullptr;            // N+1  list length of each sorted slot
+    uint64_t* lstart = nullptr;         // N    first entry of each slot's list in `lists`
+    uint16_t* lists = nullptr;
+    uint64_t list_cap = 0;
+    sph::BucketRec* bkt = nullptr;      // bucket tables, nb + 1 entries per group (last = sentinel holding nc)
+    uint64_t bkt_cap = 0;
+    sph::GroupRec* ginfo = nullptr;     // one per group
+    uint64_t ginfo_cap = 0;
+    uint32_t nc_max = 0;
+    uint64_t* offs = nullptr;           // N+1  CSR offsets, built only by sph_get_neighbours
     uint64_t n_neigh = 0;
     // scan scratch
     uint64_t* scan_status = nullptr;
@@ -141,7 +160,8 @@ int launch_sort(sph_ctx* c);                                   // sort.cu   (key
 int launch_permute(sph_ctx* c);                                // permute.cu
 int launch_tree(sph_ctx* c);                                   // tree.cu   karras + groups
 int launch_aabb(sph_ctx* c);                                   // tree.cu
-int launch_traverse(sph_ctx* c, bool fill);                    // neigh.cu
+int launch_traverse(sph_ctx* c);                               // neigh.cu  single pass: walk, test, write cache
+int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out);        // neigh.cu  group-local lists -> global CSR (getter)
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
 int launch_density(sph_ctx* c);                                // density.cu

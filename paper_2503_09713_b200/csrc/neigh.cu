@@ -1,15 +1,25 @@
 // neigh.cu -- a4: warp-cooperative, stack-based tree traversal per leaf group writing the neighbour cache
-// (Alg. 4; Alg. 5 count -> scan -> fill PAPER.md:1114-1148; two-stage idea PAPER.md:1164-1166;
-// criteria of App. E, with the cache tolerance chi, reading A2).
+// (Alg. 4; Alg. 5; two-stage idea PAPER.md:1164-1166; criteria of App. E,
+// PAPER.md:1217-1229, with the cache tolerance chi, reading A2).
 //
-// One warp per leaf group (<= 32 Morton-contiguous particles; lane = query particle). Stage 1: the warp pops up
-// to 32 nodes at a time from a shared-memory stack, each lane tests one node's box, enlarged by
-// R_kern chi max(hmax_group, hmax_node), against the group's box under the periodic minimum image (group-group
-// criterion); passing nodes with <= 32 particles become candidate buckets, larger ones push both
-// children. Stage 2: candidate buckets are staged in shared memory and every lane tests its own particle against
-// them with the exact object-object criterion d^2 < (R_kern chi max(h_a,h_b))^2. The arithmetic
-// of that test is written without FMA contraction so that the decision is bit-identical to a plain IEEE
-// evaluation.
+// One warp per leaf group (<= 32 Morton-contiguous particles; lane = query particle), ONE pass:
+//   Stage 1: the warp pops up to 32 nodes at a time from a shared-memory stack; each lane tests one node's box,
+//     enlarged by R_kern chi max(hmax_group, hmax_node), against the group's box under the periodic minimum image
+//     (group-group criterion). Passing nodes with <= 32 particles become candidate buckets (slot
+//     ranges), larger ones push both children.
+//   Stage 2: each bucket is staged in shared memory (positions and the precomputed cutoff square of every
+//     candidate) and every lane tests its own particle against it with the exact object-object criterion
+//     d^2 < (R_kern chi max(h_a,h_b))^2, written without FMA contraction so that the decision is
+//     bit-identical to a plain IEEE evaluation. (R_kern chi h)^2 is precomputed per particle: rounding, scaling
+//     by a positive constant and squaring are monotone, so max() commutes with them exactly. Buckets whose union
+//     box with the group spans at most L/2 on every periodic axis cannot wrap and take a loop without the
+//     minimum-image selects (the decision is exact).
+//   Output (the cache): the group's bucket table (its candidate array = concatenated slot ranges)
+//     and, per particle, the ascending list of 16-bit indices into that candidate array. Hits are buffered in
+//     shared memory and written out coalesced once the group is complete; space comes from two bump allocators
+//     (count -> allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed).
+//     A group whose buffers overflow (a list longer than kHitCap, more than kBktCap buckets) allocates from its
+//     exact counts and walks a second time writing directly.
 #include "common.cuh"
 
 namespace sph {
@@ -17,8 +27,12 @@ namespace sph {
 constexpr int kTravWarps = 8;            // warps per block
 constexpr int kStackCap = 512;           // stack entries per warp
 constexpr int kStackSlack = 192;         // above kStackCap - kStackSlack the warp pops one node at a time (pure DFS)
-constexpr int kBucketCap = 64;           // candidate buckets buffered before stage 2 runs
+constexpr int kPendCap = 64;             // candidate buckets buffered before stage 2 runs
+constexpr int kHitCap = 128;             // buffered hits per lane
+constexpr int kHitStride = kHitCap + 2;  // in u16: 65 words per lane row -> lanes at equal fill hit distinct banks
+constexpr int kBktCap = 126;             // buffered bucket records per group
 constexpr uint32_t kLeafBit = 0x80000000u;
+constexpr uint32_t kWrapBit = 0x80000000u;
 
 struct TravBox {
     double L[3], halfL[3];
@@ -28,8 +42,21 @@ struct TravBox {
 
 struct TravWarpSmem {
     uint32_t stack[kStackCap];
-    uint32_t blo[kBucketCap], bhi[kBucketCap];
-    double cx[32], cy[32], cz[32], ch[32];
+    uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
+    double2 cxy[32], czr[32];                 // staged candidates: {x, y}, {z, (R_kern chi h)^2}
+    BucketRec gb[kBktCap + 2];
+    uint16_t hits[32 * kHitStride];
+};
+
+struct TravOut {
+    uint32_t* cnt;
+    uint64_t* lstart;
+    uint16_t* lists;
+    uint64_t list_cap;
+    BucketRec* bkt;
+    uint64_t bkt_cap;
+    GroupRec* ginfo;
+    uint64_t ginfo_cap;
 };
 
 // separation of two intervals [alo,ahi], [blo,bhi] along one axis (0 if they overlap), minimum over periodic images
@@ -50,18 +77,167 @@ __device__ __forceinline__ double min_image(double d, double L, double halfL, in
     return d;
 }
 
-template <bool FILL>
+// per-lane / per-group traversal state
+struct GroupCtx {
+    double xq, yq, zq, rc2q;
+    double gxl, gxh, gyl, gyh, gzl, gzh, ghm;
+    bool qv;
+    uint32_t nhit;        // per lane
+    uint32_t nbk, nc;     // warp-uniform: buckets and candidates so far
+    uint16_t* lptr;       // DIRECT: this lane's list in global memory
+    BucketRec* bptr;      // DIRECT: the group's bucket table in global memory
+    bool can_write;       // DIRECT: allocation succeeded
+};
+
+template <bool DIRECT>
+__device__ __forceinline__ void record_hit(TravWarpSmem& s, GroupCtx& G, unsigned lane, uint32_t local) {
+    if (DIRECT) {
+        if (G.can_write) G.lptr[G.nhit] = (uint16_t)local;
+    } else {
+        if (G.nhit < (uint32_t)kHitCap) s.hits[lane * kHitStride + G.nhit] = (uint16_t)local;
+    }
+    ++G.nhit;
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, unsigned lane,
+                                       const double* __restrict__ x, const double* __restrict__ y,
+                                       const double* __restrict__ z, const double* __restrict__ h,
+                                       const TravBox& tb, double rk_chi) {
+    for (int b = 0; b < npend; ++b) {
+        const uint32_t plo = s.plo[b], bn = s.pn[b];
+        const uint32_t blo = plo & ~kWrapBit;
+        const bool wrap = (plo & kWrapBit) != 0u;
+        __syncwarp();                                   // readers of the previous bucket are done
+        if (lane < bn) {
+            const double hh = h[blo + lane];
+            const double rc = __dmul_rn(rk_chi, hh);
+            s.cxy[lane] = make_double2(x[blo + lane], y[blo + lane]);
+            s.czr[lane] = make_double2(z[blo + lane], __dmul_rn(rc, rc));
+        }
+        if (lane == 0) {
+            BucketRec r;
+            r.lo = blo; r.cstart = G.nc;
+            if (DIRECT) { if (G.can_write) G.bptr[G.nbk] = r; }
+            else if (G.nbk < (uint32_t)kBktCap) s.gb[G.nbk] = r;
+        }
+        __syncwarp();
+        if (!wrap) {
+#pragma unroll 4
+            for (uint32_t ci = 0; ci < bn; ++ci) {
+                const double2 a = s.cxy[ci], c = s.czr[ci];
+                const double dx = __dsub_rn(G.xq, a.x), dy = __dsub_rn(G.yq, a.y), dz = __dsub_rn(G.zq, c.x);
+                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                if (G.qv && (d2 < G.rc2q || d2 < c.y)) record_hit<DIRECT>(s, G, lane, G.nc + ci);
+            }
+        } else {
+            for (uint32_t ci = 0; ci < bn; ++ci) {
+                const double2 a = s.cxy[ci], c = s.czr[ci];
+                const double dx = min_image(__dsub_rn(G.xq, a.x), tb.L[0], tb.halfL[0], tb.periodic[0]);
+                const double dy = min_image(__dsub_rn(G.yq, a.y), tb.L[1], tb.halfL[1], tb.periodic[1]);
+                const double dz = min_image(__dsub_rn(G.zq, c.x), tb.L[2], tb.halfL[2], tb.periodic[2]);
+                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                if (G.qv && (d2 < G.rc2q || d2 < c.y)) record_hit<DIRECT>(s, G, lane, G.nc + ci);
+            }
+        }
+        G.nc += bn;
+        G.nbk += 1u;
+    }
+}
+
+// one complete walk of the tree for the group described by G
+template <bool DIRECT>
+__device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane, unsigned lt, int64_t N,
+                                     const double* __restrict__ x, const double* __restrict__ y,
+                                     const double* __restrict__ z, const double* __restrict__ h,
+                                     const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
+    G.nhit = 0u; G.nbk = 0u; G.nc = 0u;
+    int sp = 1, nb = 0;
+    __syncwarp();
+    if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
+    __syncwarp();
+    while (sp > 0) {
+        int npop = min(sp, 32);
+        if (sp > kStackCap - kStackSlack) npop = 1;
+        const bool have = (int)lane < npop;
+        const uint32_t e = have ? s.stack[sp - 1 - lane] : 0u;
+        sp -= npop;
+        __syncwarp();
+        bool pass = false, small = false, wrap = false;
+        uint32_t rlo = 0, rhi = 0, split = 0;
+        if (have) {
+            double blo[3], bhi[3], bhm;
+            if (e & kLeafBit) {
+                rlo = rhi = e & ~kLeafBit;
+                blo[0] = bhi[0] = x[rlo]; blo[1] = bhi[1] = y[rlo]; blo[2] = bhi[2] = z[rlo];
+                bhm = h[rlo];
+                small = true;
+            } else {
+                const double2* p = reinterpret_cast<const double2*>(nodes + e);
+                const double2 v0 = __ldg(p), v1 = __ldg(p + 1), v2 = __ldg(p + 2), v3 = __ldg(p + 3);
+                blo[0] = v0.x; blo[1] = v0.y; blo[2] = v1.x; bhi[0] = v1.y; bhi[1] = v2.x; bhi[2] = v2.y;
+                bhm = v3.x;
+                const long long ints = __double_as_longlong(v3.y);
+                const int32_t other = (int32_t)(ints & 0xffffffffll);
+                split = (uint32_t)(ints >> 32);
+                rlo = min(e, (uint32_t)other);
+                rhi = max(e, (uint32_t)other);
+                small = (rhi - rlo + 1) <= (uint32_t)kGroup;
+            }
+            // group-group criterion, conservative under rounding (tiny pad)
+            const double ext = rk_chi * fmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
+            pass = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]) <= ext &&
+                   axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]) <= ext &&
+                   axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]) <= ext;
+            // can any (query, candidate) separation exceed L/2 on a periodic axis? (exact: rounding is monotone)
+            wrap = (tb.periodic[0] && (fmax(G.gxh, bhi[0]) - fmin(G.gxl, blo[0]) > tb.halfL[0])) ||
+                   (tb.periodic[1] && (fmax(G.gyh, bhi[1]) - fmin(G.gyl, blo[1]) > tb.halfL[1])) ||
+                   (tb.periodic[2] && (fmax(G.gzh, bhi[2]) - fmin(G.gzl, blo[2]) > tb.halfL[2]));
+        }
+        const bool push = pass && !small, emit = pass && small;
+        const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
+        if (push) {
+            const int at = sp + 2 * __popc(pm & lt);
+            s.stack[at] = (rhi == split + 1) ? (kLeafBit | (split + 1)) : (split + 1);
+            s.stack[at + 1] = (rlo == split) ? (kLeafBit | split) : split;
+        }
+        sp += 2 * __popc(pm);
+        if (emit) {
+            const int at = nb + __popc(em & lt);
+            s.plo[at] = rlo | (wrap ? kWrapBit : 0u);
+            s.pn[at] = rhi - rlo + 1;
+        }
+        nb += __popc(em);
+        __syncwarp();
+        if (nb > kPendCap - 32) { stage2<DIRECT>(s, G, nb, lane, x, y, z, h, tb, rk_chi); nb = 0; }
+    }
+    __syncwarp();
+    stage2<DIRECT>(s, G, nb, lane, x, y, z, h, tb, rk_chi);
+    __syncwarp();
+}
+
+__device__ __forceinline__ uint32_t warp_sum_u32(uint32_t v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ uint32_t warp_max_u32(uint32_t v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
 __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
     int64_t N, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ h, const NodeRec* __restrict__ nodes, const uint32_t* __restrict__ grp_lo,
-    const DevScalars* sc_in, TravBox tb, double rk_chi, uint32_t* __restrict__ cnt,
-    const uint64_t* __restrict__ offs, uint32_t* __restrict__ nbr, uint32_t* work_counter, DevScalars* sc_out) {
+    TravBox tb, double rk_chi, TravOut out, uint32_t* work_counter, DevScalars* sc) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TravWarpSmem& s = reinterpret_cast<TravWarpSmem*>(smem_raw)[threadIdx.x >> 5];
     const unsigned lane = lane_id();
     const unsigned lt = lanemask_lt();
-    const uint32_t n_groups = sc_in->n_groups;
-    unsigned mn = 0xffffffffu, mx = 0u;
+    const uint32_t n_groups = sc->n_groups;
+    unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u, nbmax = 0u;
 
     for (;;) {
         uint32_t g = 0;
@@ -69,133 +245,104 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= n_groups) break;
         const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
-        const bool qv = lane < nq;
-        const uint32_t a = glo + (qv ? lane : 0);
-        const double xq = x[a], yq = y[a], zq = z[a], hq = h[a];
+        GroupCtx G;
+        G.qv = lane < nq;
+        const uint32_t a = glo + (G.qv ? lane : 0);
+        const double hq = h[a];
+        G.xq = x[a]; G.yq = y[a]; G.zq = z[a];
+        {
+            const double rc = __dmul_rn(rk_chi, hq);
+            G.rc2q = __dmul_rn(rc, rc);
+        }
         // group box and max h (lanes beyond nq replicate lane 0)
-        const double gxl = warp_min(xq), gxh = warp_max(xq), gyl = warp_min(yq), gyh = warp_max(yq);
-        const double gzl = warp_min(zq), gzh = warp_max(zq), ghm = warp_max(hq);
-        uint32_t n_found = 0;
-        uint64_t wofs = 0;
-        if (FILL) wofs = offs[a];
+        G.gxl = warp_min(G.xq); G.gxh = warp_max(G.xq); G.gyl = warp_min(G.yq); G.gyh = warp_max(G.yq);
+        G.gzl = warp_min(G.zq); G.gzh = warp_max(G.zq); G.ghm = warp_max(hq);
+        G.lptr = nullptr; G.bptr = nullptr; G.can_write = false;
 
-        int sp = 0, nb = 0;
-        if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
-        sp = 1;
-        __syncwarp();
+        walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
-        auto stage2 = [&]() {
-            for (int b = 0; b < nb; ++b) {
-                const uint32_t blo = s.blo[b], bn = s.bhi[b] - blo + 1;
-                __syncwarp();
-                if (lane < bn) {
-                    s.cx[lane] = x[blo + lane]; s.cy[lane] = y[blo + lane];
-                    s.cz[lane] = z[blo + lane]; s.ch[lane] = h[blo + lane];
-                }
-                __syncwarp();
-                if (qv) {
-                    for (uint32_t cidx = 0; cidx < bn; ++cidx) {
-                        double dx = min_image(__dsub_rn(xq, s.cx[cidx]), tb.L[0], tb.halfL[0], tb.periodic[0]);
-                        double dy = min_image(__dsub_rn(yq, s.cy[cidx]), tb.L[1], tb.halfL[1], tb.periodic[1]);
-                        double dz = min_image(__dsub_rn(zq, s.cz[cidx]), tb.L[2], tb.halfL[2], tb.periodic[2]);
-                        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                        double rc = __dmul_rn(rk_chi, fmax(hq, s.ch[cidx]));
-                        if (d2 < __dmul_rn(rc, rc)) {
-                            if (FILL) nbr[wofs + n_found] = blo + cidx;
-                            ++n_found;
-                        }
-                    }
-                }
-            }
-            nb = 0;
-        };
-
-        while (sp > 0) {
-            int npop = min(sp, 32);
-            if (sp > kStackCap - kStackSlack) npop = 1;
-            bool have = (int)lane < npop;
-            uint32_t e = have ? s.stack[sp - 1 - lane] : 0u;
-            sp -= npop;
-            __syncwarp();
-            bool pass = false, small = false;
-            uint32_t rlo = 0, rhi = 0, split = 0;
-            if (have) {
-                double blo[3], bhi[3], bhm;
-                if (e & kLeafBit) {
-                    rlo = rhi = e & ~kLeafBit;
-                    blo[0] = bhi[0] = x[rlo]; blo[1] = bhi[1] = y[rlo]; blo[2] = bhi[2] = z[rlo];
-                    bhm = h[rlo];
-                    small = true;
-                } else {
-                    const double2* p = reinterpret_cast<const double2*>(nodes + e);
-                    double2 v0 = __ldg(p), v1 = __ldg(p + 1), v2 = __ldg(p + 2), v3 = __ldg(p + 3);
-                    blo[0] = v0.x; blo[1] = v0.y; blo[2] = v1.x; bhi[0] = v1.y; bhi[1] = v2.x; bhi[2] = v2.y;
-                    bhm = v3.x;
-                    long long ints = __double_as_longlong(v3.y);
-                    int32_t other = (int32_t)(ints & 0xffffffffll);
-                    split = (uint32_t)(ints >> 32);
-                    rlo = min(e, (uint32_t)other);
-                    rhi = max(e, (uint32_t)other);
-                    small = (rhi - rlo + 1) <= (uint32_t)kGroup;
-                }
-                // group-group criterion, conservative under rounding (tiny pad)
-                double ext = rk_chi * fmax(ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
-                pass = axis_gap(gxl, gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]) <= ext &&
-                       axis_gap(gyl, gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]) <= ext &&
-                       axis_gap(gzl, gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]) <= ext;
-            }
-            const bool push = pass && !small, emit = pass && small;
-            const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
-            if (push) {
-                int at = sp + 2 * __popc(pm & lt);
-                s.stack[at] = (rhi == split + 1) ? (kLeafBit | (split + 1)) : (split + 1);
-                s.stack[at + 1] = (rlo == split) ? (kLeafBit | split) : split;
-            }
-            sp += 2 * __popc(pm);
-            if (emit) {
-                int at = nb + __popc(em & lt);
-                s.blo[at] = rlo;
-                s.bhi[at] = rhi;
-            }
-            nb += __popc(em);
-            __syncwarp();
-            if (nb > kBucketCap - 32) stage2();
-        }
-        __syncwarp();
-        stage2();
-
-        if (!FILL) {
-            if (qv) {
-                cnt[a] = n_found;
-                mn = min(mn, n_found);
-                mx = max(mx, n_found);
-            }
-        }
-    }
-    if (!FILL) {
+        // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and bucket table ----
+        const uint32_t nhit = G.qv ? G.nhit : 0u;
+        const uint32_t nbk = G.nbk, nc = G.nc;
+        uint32_t incl = nhit;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
-            mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (unsigned)o) incl += t;
         }
-        if (lane == 0 && mx >= mn) {
-            atomicMin(&sc_out->nbr_min, mn);
-            atomicMax(&sc_out->nbr_max, mx);
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+        const uint32_t maxhit = warp_max_u32(nhit);
+        unsigned long long lbase = 0, bbase = 0;
+        if (lane == 0) {
+            lbase = atomicAdd(&sc->list_cursor, (unsigned long long)((total + 7u) & ~7u));
+            bbase = atomicAdd(&sc->bkt_cursor, (unsigned long long)(nbk + 1u));
+            atomicAdd(&sc->n_neigh, (unsigned long long)total);
         }
+        lbase = __shfl_sync(0xffffffffu, lbase, 0);
+        bbase = __shfl_sync(0xffffffffu, bbase, 0);
+        const bool fits = (lbase + ((total + 7u) & ~7u) <= out.list_cap) && (bbase + nbk + 1u <= out.bkt_cap) &&
+                          ((uint64_t)g < out.ginfo_cap) && (nc <= 65535u);
+        const uint64_t my_start = lbase + (incl - nhit);
+        if (G.qv) {
+            out.cnt[a] = nhit;
+            out.lstart[a] = my_start;
+        }
+        if (fits) {
+            if (lane == 0) {
+                GroupRec r;
+                r.bkt_off_lo = (uint32_t)(bbase & 0xffffffffull); r.bkt_off_hi = (uint32_t)(bbase >> 32);
+                r.nb = nbk; r.nc = nc;
+                out.ginfo[g] = r;
+                BucketRec sentinel; sentinel.lo = 0u; sentinel.cstart = nc;
+                out.bkt[bbase + nbk] = sentinel;
+            }
+            const bool overflow = (maxhit > (uint32_t)kHitCap) || (nbk > (uint32_t)kBktCap);
+            if (!overflow) {
+                for (uint32_t j = lane; j < nbk; j += 32) out.bkt[bbase + j] = s.gb[j];
+                // lists: the warp copies one particle's buffered list at a time (coalesced 16-bit stores)
+                for (uint32_t p = 0; p < nq; ++p) {
+                    const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
+                    const uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - np);
+                    for (uint32_t k = lane; k < np; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
+                }
+            } else {
+                // fallback: second walk writing directly at the now-known positions
+                G.lptr = out.lists + my_start;
+                G.bptr = out.bkt + bbase;
+                G.can_write = true;
+                walk<true>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
+                if (lane == 0) atomicAdd(&sc->n_fallback, 1u);
+            }
+        }
+        if (nc > 65535u && lane == 0) atomicAdd(&sc->n_cand_overflow, 1u);
+        if (G.qv) { mn = min(mn, nhit); mx = max(mx, nhit); }
+        ncmax = max(ncmax, nc);
+        nbmax = max(nbmax, nbk);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if (lane == 0) {
+        if (mx >= mn) { atomicMin(&sc->nbr_min, mn); atomicMax(&sc->nbr_max, mx); }
+        atomicMax(&sc->nc_max, ncmax);
+        atomicMax(&sc->nb_max, nbmax);
     }
 }
 
-__global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc, int reset_minmax) {
+__global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc) {
     *work_counter = 0u;
-    if (reset_minmax) { sc->nbr_min = 0xffffffffu; sc->nbr_max = 0u; }
+    sc->nbr_min = 0xffffffffu; sc->nbr_max = 0u;
+    sc->list_cursor = 0ull; sc->bkt_cursor = 0ull; sc->n_neigh = 0ull;
+    sc->nc_max = 0u; sc->nb_max = 0u; sc->n_cand_overflow = 0u; sc->n_fallback = 0u;
 }
 
-int launch_traverse(sph_ctx* c, bool fill) {
+int launch_traverse(sph_ctx* c) {
     static bool attr_set = false;
     const int smem = (int)sizeof(TravWarpSmem) * kTravWarps;
     if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_traverse<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SPH_CUDA(c, cudaFuncSetAttribute(k_traverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SPH_CUDA(c, cudaFuncSetAttribute(k_traverse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     TravBox tb;
@@ -208,21 +355,50 @@ int launch_traverse(sph_ctx* c, bool fill) {
     }
     tb.gg_pad = 1e-14 * Lmax;
     const double rk_chi = kRkern * c->p.chi;
+    TravOut out;
+    out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
+    out.bkt = c->bkt; out.bkt_cap = c->bkt_cap; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
     uint32_t* wc = c->sort_counters + 8;   // spare counter word
-    k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc, fill ? 0 : 1);
-    // persistent grid: enough warps to fill the machine, work handed out through an atomic counter
-    int64_t warps_needed = (c->N + 31) / 32;   // upper bound on useful warps is the group count <= N
-    unsigned blocks = (unsigned)min((int64_t)148 * 6, (warps_needed + kTravWarps - 1) / kTravWarps);
+    k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc);
+    // persistent grid: two CTAs per SM (shared-memory bound), work handed out through an atomic counter
+    const int64_t warps_needed = (c->N + 31) / 32;
+    unsigned blocks = (unsigned)min((int64_t)148 * 2, (warps_needed + kTravWarps - 1) / kTravWarps);
     if (blocks == 0) blocks = 1;
-    if (fill)
-        k_traverse<true><<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h,
-                                                                       c->nodes, c->grp_lo, c->d_sc, tb, rk_chi, c->cnt,
-                                                                       c->offs, c->nbr, wc, c->d_sc);
-    else
-        k_traverse<false><<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h,
-                                                                        c->nodes, c->grp_lo, c->d_sc, tb, rk_chi, c->cnt,
-                                                                        c->offs, c->nbr, wc, c->d_sc);
+    k_traverse<<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
+                                                             c->grp_lo, tb, rk_chi, out, wc, c->d_sc);
     c->launches += 2;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+// ---- getter path: group-local lists -> global CSR over sorted slots (sph_get_neighbours) ----
+__global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t* __restrict__ gscan,
+                                                      const GroupRec* __restrict__ ginfo,
+                                                      const BucketRec* __restrict__ bkt,
+                                                      const uint32_t* __restrict__ cnt,
+                                                      const uint64_t* __restrict__ lstart,
+                                                      const uint16_t* __restrict__ lists,
+                                                      const uint64_t* __restrict__ offs, uint32_t* __restrict__ idx) {
+    const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    const uint32_t g = gscan[a + 1] - 1u;          // gscan = exclusive scan of the group-start flags
+    const GroupRec gr = ginfo[g];
+    const BucketRec* tab = bkt + (((uint64_t)gr.bkt_off_hi << 32) | gr.bkt_off_lo);
+    const uint16_t* li = lists + lstart[a];
+    const uint32_t n = cnt[a];
+    uint32_t j = 0;
+    uint64_t o = offs[a];
+    for (uint32_t k = 0; k < n; ++k) {
+        const uint32_t cl = li[k];
+        while (tab[j + 1].cstart <= cl) ++j;       // lists ascend, so the bucket pointer only moves forward
+        idx[o + k] = tab[j].lo + (cl - tab[j].cstart);
+    }
+}
+
+int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out) {
+    k_cache_to_csr<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->bkt, c->cnt, c->lstart,
+                                                             c->lists, c->offs, idx_out);
+    c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }
