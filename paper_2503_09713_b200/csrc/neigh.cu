@@ -28,8 +28,9 @@ constexpr int kTravWarps = 8;            // warps per block
 constexpr int kStackCap = 512;           // stack entries per warp
 constexpr int kStackSlack = 192;         // above kStackCap - kStackSlack the warp pops one node at a time (pure DFS)
 constexpr int kPendCap = 64;             // candidate buckets buffered before stage 2 runs
-constexpr int kHitCap = 128;             // buffered hits per lane
-constexpr int kHitStride = kHitCap + 2;  // in u16: 65 words per lane row -> lanes at equal fill hit distinct banks
+constexpr int kHitCap = 112;             // buffered hits per lane
+constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
+constexpr int kHitStride = kHitCap + kHitSlack + 2;   // in u16: 73 words per lane row (odd: rows start in distinct banks)
 constexpr int kBktCap = 126;             // buffered bucket records per group
 constexpr uint32_t kLeafBit = 0x80000000u;
 constexpr uint32_t kWrapBit = 0x80000000u;
@@ -43,7 +44,8 @@ struct TravBox {
 struct TravWarpSmem {
     uint32_t stack[kStackCap];
     uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
-    double2 cxy[32], czr[32];                 // staged candidates: {x, y}, {z, (R_kern chi h)^2}
+    double2 cxy[32], czr[32];                 // staged candidates (compacted): {x, y}, {z, (R_kern chi h)^2}
+    uint32_t cid[32];                         // their indices in the group's candidate array
     BucketRec gb[kBktCap + 2];
     uint16_t hits[32 * kHitStride];
 };
@@ -81,39 +83,81 @@ __device__ __forceinline__ double min_image(double d, double L, double halfL, in
 struct GroupCtx {
     double xq, yq, zq, rc2q;
     double gxl, gxh, gyl, gyh, gzl, gzh, ghm;
-    bool qv;
-    uint32_t nhit;        // per lane
+    double rc2g;          // (R_kern chi hmax_group)^2, for the per-candidate prefilter
+    uint32_t nhit;        // per lane: hits so far (exact)
+    uint32_t wpos;        // per lane, buffered mode: store position in the lane's row (clamped to kHitCap per bucket)
     uint32_t nbk, nc;     // warp-uniform: buckets and candidates so far
     uint16_t* lptr;       // DIRECT: this lane's list in global memory
     BucketRec* bptr;      // DIRECT: the group's bucket table in global memory
     bool can_write;       // DIRECT: allocation succeeded
 };
 
-template <bool DIRECT>
-__device__ __forceinline__ void record_hit(TravWarpSmem& s, GroupCtx& G, unsigned lane, uint32_t local) {
-    if (DIRECT) {
-        if (G.can_write) G.lptr[G.nhit] = (uint16_t)local;
-    } else {
-        if (G.nhit < (uint32_t)kHitCap) s.hits[lane * kHitStride + G.nhit] = (uint16_t)local;
-    }
-    ++G.nhit;
+// d2 < a || d2 < b as two predicate-combining compares (the compiler otherwise builds a NaN-safe fp64 max)
+__device__ __forceinline__ bool lt_either(double d2, double a, double b) {
+    int r;
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tsetp.lt.or.f64 p, %1, %3, p;\n\tselp.s32 %0, 1, 0, p;\n\t}"
+        : "=r"(r) : "d"(d2), "d"(a), "d"(b));
+    return r != 0;
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, unsigned lane,
+__device__ __forceinline__ void record_hit(GroupCtx& G, uint32_t& wp, uint32_t local) {
+    if (DIRECT) {
+        if (G.can_write) G.lptr[G.nhit] = (uint16_t)local;
+        ++G.nhit;
+    } else {
+        // wp = 32-bit shared-memory address of the lane's next free entry; the row has kHitSlack entries
+        // beyond kHitCap, so no capacity check is needed inside a bucket
+        asm volatile("st.shared.u16 [%0], %1;" :: "r"(wp), "h"((unsigned short)local) : "memory");
+        wp += 2u;
+    }
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, unsigned lane, unsigned lt,
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const TravBox& tb, double rk_chi) {
+    const uint32_t row = lane * kHitStride;
+    // software pipeline: the next bucket's candidate (one per lane) is in flight while this one is tested
+    double px = 0.0, py = 0.0, pz = 0.0, ph = 0.0;
+    if (npend > 0) {
+        const uint32_t blo = s.plo[0] & ~kWrapBit;
+        if (lane < s.pn[0]) { px = x[blo + lane]; py = y[blo + lane]; pz = z[blo + lane]; ph = h[blo + lane]; }
+    }
     for (int b = 0; b < npend; ++b) {
         const uint32_t plo = s.plo[b], bn = s.pn[b];
         const uint32_t blo = plo & ~kWrapBit;
         const bool wrap = (plo & kWrapBit) != 0u;
+        const double cx = px, cy = py, cz = pz;
+        const double rc = __dmul_rn(rk_chi, ph);
+        const double rc2 = __dmul_rn(rc, rc);
+        if (b + 1 < npend) {
+            const uint32_t nlo = s.plo[b + 1] & ~kWrapBit;
+            if (lane < s.pn[b + 1]) { px = x[nlo + lane]; py = y[nlo + lane]; pz = z[nlo + lane]; ph = h[nlo + lane]; }
+        }
+        // per-candidate prefilter (one lane per candidate): squared distance from the candidate to the group's
+        // box against the larger of its own and the group's cutoff, with a relative margin far above rounding.
+        // Buckets that may wrap keep every candidate.
+        bool keep = lane < bn;
+        if (keep && !wrap) {
+            const double gx = fmax(fmax(G.gxl - cx, cx - G.gxh), 0.0);
+            const double gy = fmax(fmax(G.gyl - cy, cy - G.gyh), 0.0);
+            const double gz = fmax(fmax(G.gzl - cz, cz - G.gzh), 0.0);
+            keep = gx * gx + gy * gy + gz * gz <= fmax(rc2, G.rc2g) * (1.0 + 1e-9);
+        }
+        const unsigned km = __ballot_sync(0xffffffffu, keep);
+        const uint32_t nk = (uint32_t)__popc(km), nk4 = (nk + 3u) & ~3u, pos = (uint32_t)__popc(km & lt);
         __syncwarp();                                   // readers of the previous bucket are done
-        if (lane < bn) {
-            const double hh = h[blo + lane];
-            const double rc = __dmul_rn(rk_chi, hh);
-            s.cxy[lane] = make_double2(x[blo + lane], y[blo + lane]);
-            s.czr[lane] = make_double2(z[blo + lane], __dmul_rn(rc, rc));
+        if (keep) {
+            s.cxy[pos] = make_double2(cx, cy);
+            s.czr[pos] = make_double2(cz, rc2);
+            s.cid[pos] = G.nc + lane;                   // index in the group's candidate array
+        }
+        if (lane < 4u && nk + lane < nk4) {             // pad to a multiple of four with candidates nobody can hit
+            s.cxy[nk + lane] = make_double2(1e300, 1e300);
+            s.czr[nk + lane] = make_double2(1e300, 0.0);
+            s.cid[nk + lane] = 0u;
         }
         if (lane == 0) {
             BucketRec r;
@@ -122,23 +166,35 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             else if (G.nbk < (uint32_t)kBktCap) s.gb[G.nbk] = r;
         }
         __syncwarp();
+        const uint32_t w0 = (uint32_t)__cvta_generic_to_shared(&s.hits[row + G.wpos]);
+        uint32_t wp = w0;
         if (!wrap) {
-#pragma unroll 4
-            for (uint32_t ci = 0; ci < bn; ++ci) {
-                const double2 a = s.cxy[ci], c = s.czr[ci];
-                const double dx = __dsub_rn(G.xq, a.x), dy = __dsub_rn(G.yq, a.y), dz = __dsub_rn(G.zq, c.x);
-                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                if (G.qv && (d2 < G.rc2q || d2 < c.y)) record_hit<DIRECT>(s, G, lane, G.nc + ci);
+            for (uint32_t ci = 0; ci < nk4; ci += 4) {
+                const uint4 id4 = *reinterpret_cast<const uint4*>(&s.cid[ci]);
+                const uint32_t ids[4] = {id4.x, id4.y, id4.z, id4.w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const double2 a = s.cxy[ci + u], c = s.czr[ci + u];
+                    const double dx = __dsub_rn(G.xq, a.x), dy = __dsub_rn(G.yq, a.y), dz = __dsub_rn(G.zq, c.x);
+                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    if (lt_either(d2, G.rc2q, c.y)) record_hit<DIRECT>(G, wp, ids[u]);
+                }
             }
         } else {
-            for (uint32_t ci = 0; ci < bn; ++ci) {
+            for (uint32_t ci = 0; ci < nk; ++ci) {
                 const double2 a = s.cxy[ci], c = s.czr[ci];
                 const double dx = min_image(__dsub_rn(G.xq, a.x), tb.L[0], tb.halfL[0], tb.periodic[0]);
                 const double dy = min_image(__dsub_rn(G.yq, a.y), tb.L[1], tb.halfL[1], tb.periodic[1]);
                 const double dz = min_image(__dsub_rn(G.zq, c.x), tb.L[2], tb.halfL[2], tb.periodic[2]);
                 const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                if (G.qv && (d2 < G.rc2q || d2 < c.y)) record_hit<DIRECT>(s, G, lane, G.nc + ci);
+                if (lt_either(d2, G.rc2q, c.y)) record_hit<DIRECT>(G, wp, s.cid[ci]);
             }
+        }
+        if (!DIRECT) {
+            const uint32_t got = (wp - w0) >> 1;
+            G.nhit += got;
+            G.wpos += got;
+            if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;   // overflowed row: keep counting, stop growing
         }
         G.nc += bn;
         G.nbk += 1u;
@@ -151,7 +207,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.nbk = 0u; G.nc = 0u;
+    G.nhit = 0u; G.wpos = 0u; G.nbk = 0u; G.nc = 0u;
     int sp = 1, nb = 0;
     __syncwarp();
     if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
@@ -186,9 +242,10 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
             }
             // group-group criterion, conservative under rounding (tiny pad)
             const double ext = rk_chi * fmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
-            pass = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]) <= ext &&
-                   axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]) <= ext &&
-                   axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]) <= ext;
+            const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
+            const double ggy = axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]);
+            const double ggz = axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]);
+            pass = ggx * ggx + ggy * ggy + ggz * ggz <= ext * ext;
             // can any (query, candidate) separation exceed L/2 on a periodic axis? (exact: rounding is monotone)
             wrap = (tb.periodic[0] && (fmax(G.gxh, bhi[0]) - fmin(G.gxl, blo[0]) > tb.halfL[0])) ||
                    (tb.periodic[1] && (fmax(G.gyh, bhi[1]) - fmin(G.gyl, blo[1]) > tb.halfL[1])) ||
@@ -209,10 +266,10 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
         }
         nb += __popc(em);
         __syncwarp();
-        if (nb > kPendCap - 32) { stage2<DIRECT>(s, G, nb, lane, x, y, z, h, tb, rk_chi); nb = 0; }
+        if (nb > kPendCap - 32) { stage2<DIRECT>(s, G, nb, lane, lt, x, y, z, h, tb, rk_chi); nb = 0; }
     }
     __syncwarp();
-    stage2<DIRECT>(s, G, nb, lane, x, y, z, h, tb, rk_chi);
+    stage2<DIRECT>(s, G, nb, lane, lt, x, y, z, h, tb, rk_chi);
     __syncwarp();
 }
 
@@ -246,8 +303,8 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         if (g >= n_groups) break;
         const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
         GroupCtx G;
-        G.qv = lane < nq;
-        const uint32_t a = glo + (G.qv ? lane : 0);
+        const bool qv = lane < nq;
+        const uint32_t a = glo + (qv ? lane : 0);
         const double hq = h[a];
         G.xq = x[a]; G.yq = y[a]; G.zq = z[a];
         {
@@ -257,12 +314,17 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         // group box and max h (lanes beyond nq replicate lane 0)
         G.gxl = warp_min(G.xq); G.gxh = warp_max(G.xq); G.gyl = warp_min(G.yq); G.gyh = warp_max(G.yq);
         G.gzl = warp_min(G.zq); G.gzh = warp_max(G.zq); G.ghm = warp_max(hq);
+        {
+            const double rcg = __dmul_rn(rk_chi, G.ghm);
+            G.rc2g = __dmul_rn(rcg, rcg);
+        }
+        if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
         G.lptr = nullptr; G.bptr = nullptr; G.can_write = false;
 
         walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
         // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and bucket table ----
-        const uint32_t nhit = G.qv ? G.nhit : 0u;
+        const uint32_t nhit = qv ? G.nhit : 0u;
         const uint32_t nbk = G.nbk, nc = G.nc;
         uint32_t incl = nhit;
 #pragma unroll
@@ -283,7 +345,7 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         const bool fits = (lbase + ((total + 7u) & ~7u) <= out.list_cap) && (bbase + nbk + 1u <= out.bkt_cap) &&
                           ((uint64_t)g < out.ginfo_cap) && (nc <= 65535u);
         const uint64_t my_start = lbase + (incl - nhit);
-        if (G.qv) {
+        if (qv) {
             out.cnt[a] = nhit;
             out.lstart[a] = my_start;
         }
@@ -315,7 +377,7 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
             }
         }
         if (nc > 65535u && lane == 0) atomicAdd(&sc->n_cand_overflow, 1u);
-        if (G.qv) { mn = min(mn, nhit); mx = max(mx, nhit); }
+        if (qv) { mn = min(mn, nhit); mx = max(mx, nhit); }
         ncmax = max(ncmax, nc);
         nbmax = max(nbmax, nbk);
     }
