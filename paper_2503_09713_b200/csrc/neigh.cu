@@ -90,6 +90,7 @@ struct GroupCtx {
     uint16_t* lptr;       // DIRECT: this lane's list in global memory
     BucketRec* bptr;      // DIRECT: the group's bucket table in global memory
     bool can_write;       // DIRECT: allocation succeeded
+    bool anywrap;         // warp-uniform: some bucket of this group may wrap around a periodic axis
 };
 
 // d2 < a || d2 < b as two predicate-combining compares (the compiler otherwise builds a NaN-safe fp64 max)
@@ -129,6 +130,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
         const uint32_t plo = s.plo[b], bn = s.pn[b];
         const uint32_t blo = plo & ~kWrapBit;
         const bool wrap = (plo & kWrapBit) != 0u;
+        G.anywrap |= wrap;
         const double cx = px, cy = py, cz = pz;
         const double rc = __dmul_rn(rk_chi, ph);
         const double rc2 = __dmul_rn(rc, rc);
@@ -207,7 +209,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.nbk = 0u; G.nc = 0u;
+    G.nhit = 0u; G.wpos = 0u; G.nbk = 0u; G.nc = 0u; G.anywrap = false;
     int sp = 1, nb = 0;
     __syncwarp();
     if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
@@ -353,7 +355,7 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
             if (lane == 0) {
                 GroupRec r;
                 r.bkt_off_lo = (uint32_t)(bbase & 0xffffffffull); r.bkt_off_hi = (uint32_t)(bbase >> 32);
-                r.nb = nbk; r.nc = nc;
+                r.nb = nbk; r.nc = nc | (G.anywrap ? 0x80000000u : 0u);
                 out.ginfo[g] = r;
                 BucketRec sentinel; sentinel.lo = 0u; sentinel.cstart = nc;
                 out.bkt[bbase + nbk] = sentinel;
