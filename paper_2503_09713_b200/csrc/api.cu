@@ -91,6 +91,10 @@ __global__ void k_iota(int64_t N, uint32_t* id) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) id[i] = (uint32_t)i;
 }
+__global__ void k_mass_uniform(int64_t N, const double* __restrict__ m, DevScalars* sc) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N && m[i] != m[0]) sc->mass_nonuniform = 1u;
+}
 __global__ void k_fill(int64_t N, double* p, double v) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) p[i] = v;
@@ -260,7 +264,11 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
         k_h0_fallback<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, mtot, vol, c->p.hfact, c->cur.h);
         c->launches += 2;
     }
+    k_mass_uniform<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, c->d_sc);
+    c->launches++;
     SPH_CUDA(c, cudaGetLastError());
+    SPH_TRY(read_scalars(c));
+    c->uniform_mass = (c->h_sc->mass_nonuniform == 0u);
     c->state = S_FIELDS;
     if (run_white_step) {
         SPH_TRY(sph_build_tree(c));

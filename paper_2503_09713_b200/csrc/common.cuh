@@ -65,6 +65,7 @@ struct DevScalars {
     unsigned int nc_max;             // largest candidate count of any group
     unsigned int nb_max;             // largest bucket count of any group
     unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
+    unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
 };
 
@@ -129,6 +130,7 @@ struct sph_ctx {
     double t = 0.0;
     int64_t launches = 0;
     bool have_cfl_dt = false;
+    bool uniform_mass = false;          // all particle masses equal (density kernel variant)
 
     std::vector<sph::TimerRec> timers;
     std::vector<cudaEvent_t> event_pool;

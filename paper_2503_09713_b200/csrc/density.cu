@@ -42,21 +42,25 @@ __device__ __forceinline__ double octet_sum(double v) {
 struct DensPar { double hfact, chi, lambda, eps_h; int max_iter; };
 struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 
-template <bool WRAP>
+// UNIM: every candidate of the group has the same mass (checked while staging): the mass factors out of the sums
+// and the per-neighbour mass registers disappear.
+template <bool WRAP, bool UNIM>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
                                             const uint16_t* __restrict__ li, int n, unsigned sl,
                                             const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
-    double r[kRegChunks], mb[kRegChunks];
+    double r[kRegChunks], mb[UNIM ? 1 : kRegChunks];
+    const double m0 = sm[0];
 #pragma unroll
     for (int c = 0; c < kRegChunks; ++c) {
         const int k = c * 8 + (int)sl;
-        r[c] = 0.0; mb[c] = 0.0;
+        r[c] = 1e100;                                  // q >> 2 (finite): outside the kernel support, contributes 0
+        if (!UNIM) mb[c] = 0.0;
         if (k < n) {
             const uint32_t b = li[k];
             r[c] = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db);
-            mb[c] = sm[b];
+            if (!UNIM) mb[c] = sm[b];
         }
     }
     // sums over the list at smoothing length h: rs = sum m f(q), ss = sum m (3 f + q f')
@@ -67,20 +71,25 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         for (int c = 0; c < kRegChunks; ++c) {
             double qq = r[c] * hinv, f, df;
             m4(qq, f, df);
-            rs = fma(mb[c], f, rs);
-            ss = fma(mb[c], fma(qq, df, 3.0 * f), ss);
+            if (UNIM) {
+                rs += f;
+                ss += fma(qq, df, 3.0 * f);
+            } else {
+                rs = fma(mb[c], f, rs);
+                ss = fma(mb[c], fma(qq, df, 3.0 * f), ss);
+            }
         }
         for (int k = kRegChunks * 8 + (int)sl; k < n; k += 8) {      // long lists: re-gather from smem
             const uint32_t b = li[k];
             double qq = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, df;
-            const double mm = sm[b];
+            const double mm = UNIM ? 1.0 : sm[b];
             m4(qq, f, df);
             rs = fma(mm, f, rs);
             ss = fma(mm, fma(qq, df, 3.0 * f), ss);
         }
         rs = octet_sum(rs);
         ss = octet_sum(ss);
-        const double c3 = kCnorm * hinv * hinv * hinv;
+        const double c3 = (UNIM ? m0 : 1.0) * kCnorm * hinv * hinv * hinv;
         rho_sum = c3 * rs;            // Eq. 1-2
         S = -c3 * hinv * ss;          // sum_b m_b dW/dh
     };
@@ -122,7 +131,8 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     out.it = it;
 }
 
-__global__ void __launch_bounds__(kDensWarps * 32, 2) k_density(
+template <bool UNIM>
+__global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
     const GroupRec* __restrict__ ginfo, const BucketRec* __restrict__ bkt, const uint32_t* __restrict__ cnt,
@@ -161,8 +171,8 @@ __global__ void __launch_bounds__(kDensWarps * 32, 2) k_density(
     __syncthreads();
 
     DensOut o;
-    if (gwrap) octet_solve<true>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
-    else octet_solve<false>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
+    if (gwrap) octet_solve<true, UNIM>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
+    else octet_solve<false, UNIM>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
 
     if (pv && sl == 0u) {
         hout[a] = o.h;
@@ -186,7 +196,8 @@ __global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noco
 int launch_density(sph_ctx* c) {
     static bool attr_set = false;
     if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        SPH_CUDA(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        SPH_CUDA(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_set = true;
     }
     DensBox db;
@@ -203,9 +214,15 @@ int launch_density(sph_ctx* c) {
         return fail(c, SPH_ERR_CAP, "a leaf group has %u candidates: more than the density kernel can stage (%d)",
                     c->nc_max, 227 * 1024 / 32);
     k_density_reset<<<1, 1, 0, c->stream>>>(c->d_sc);
-    k_density<<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-        c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->bkt, c->cnt, c->lstart, c->lists, db,
-        dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
+    // all masses equal (checked once at init): the kernel variant without per-neighbour mass registers
+    if (c->uniform_mass)
+        k_density<true><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->bkt, c->cnt, c->lstart, c->lists, db,
+            dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
+    else
+        k_density<false><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->bkt, c->cnt, c->lstart, c->lists, db,
+            dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
     c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
