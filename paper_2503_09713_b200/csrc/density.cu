@@ -32,6 +32,14 @@ __device__ __forceinline__ double sep_r(double xa, double ya, double za, const d
     return sqrt(dx * dx + dy * dy + dz * dz);
 }
 
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
 __device__ __forceinline__ double octet_sum(double v) {
     v += __shfl_xor_sync(0xffffffffu, v, 4);
     v += __shfl_xor_sync(0xffffffffu, v, 2);
@@ -46,8 +54,8 @@ struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 // and the per-neighbour mass registers disappear.
 template <bool WRAP, bool UNIM>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
-                                            const uint16_t* __restrict__ li, int n, unsigned sl,
-                                            const double* __restrict__ sx, const double* __restrict__ sy,
+                                            const uint16_t* __restrict__ li, const uint32_t (&idx)[kRegChunks / 2],
+                                            int n, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
     double r[kRegChunks], mb[UNIM ? 1 : kRegChunks];
@@ -58,7 +66,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         r[c] = 1e100;                                  // q >> 2 (finite): outside the kernel support, contributes 0
         if (!UNIM) mb[c] = 0.0;
         if (k < n) {
-            const uint32_t b = li[k];
+            const uint32_t b = (idx[c >> 1] >> (16 * (c & 1))) & 0xffffu;
             r[c] = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db);
             if (!UNIM) mb[c] = sm[b];
         }
@@ -165,14 +173,24 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
         const uint32_t bn = tab[j + 1].cstart - b0.cstart;
         if (lane < bn) {
             const uint32_t s = b0.lo + lane, c = b0.cstart + lane;
-            sx[c] = x[s]; sy[c] = y[s]; sz[c] = z[s]; sm[c] = m[s];
+            cp_async8(sx + c, x + s); cp_async8(sy + c, y + s); cp_async8(sz + c, z + s); cp_async8(sm + c, m + s);
         }
     }
+    // the first 96 list entries of the octet's particle (two 16-bit indices per register), in flight together with
+    // the staging copies
+    uint32_t idx[kRegChunks / 2];
+#pragma unroll
+    for (int c = 0; c < kRegChunks; c += 2) {
+        const int k0 = c * 8 + (int)sl, k1 = k0 + 8;
+        const uint32_t i0 = (k0 < n) ? (uint32_t)li[k0] : 0u, i1 = (k1 < n) ? (uint32_t)li[k1] : 0u;
+        idx[c >> 1] = i0 | (i1 << 16);
+    }
+    cp_async_wait_all();
     __syncthreads();
 
     DensOut o;
-    if (gwrap) octet_solve<true, UNIM>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
-    else octet_solve<false, UNIM>(xa, ya, za, ma, h0, pv, li, n, sl, sx, sy, sz, sm, db, dp, o);
+    if (gwrap) octet_solve<true, UNIM>(xa, ya, za, ma, h0, pv, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    else octet_solve<false, UNIM>(xa, ya, za, ma, h0, pv, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
 
     if (pv && sl == 0u) {
         hout[a] = o.h;
