@@ -32,7 +32,23 @@ UNIT = "particle-updates/s"
 FLOP_PER_PAIR_DENSITY_GATHER = 11     # separation, d^2, sqrt (once per pair per density solve)
 FLOP_PER_PAIR_DENSITY_SWEEP = 16      # q, f, f', two accumulations (per pair per Newton sweep)
 FLOP_PER_PAIR_FORCE = 93              # Eq. 3-6, 8-10 per pair
-FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair (count + fill = 2 tests)
+FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair (single pass)
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
+# workload (profiles/r1_ncu_full_v5.md); only quoted when bench runs that workload
+NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.02e9, "traverse": 3.87e9, "density": 4.27e9}
+
+
+def reduce_over_ranks(ms_local: float, n_local: float, world: int, device):
+    """Whole-job aggregate: max over ranks of the device time, sum over ranks of the particles stepped."""
+    import torch
+    import torch.distributed as dist
+    tmax = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    ntot = torch.tensor([float(n_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ntot, op=dist.ReduceOp.SUM)
+    return float(tmax.item()), float(ntot.item())
 
 
 def make_workload(name: str, seed_offset: int = 0):
@@ -105,7 +121,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_side = 40
+    n_side = args.ref_side
     rate, s_per_step, n, _ = oracle_step_rate(n_side, args.steps, args.warmup)
     sample = f"C2 recipe at {n_side}^3 = {n} particles (bounded sample of the 256^3 workload), {args.steps} full oracle steps"
     line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -128,6 +144,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ref-side", type=int, default=40, help="lattice side of the oracle's bounded sample")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -176,12 +193,7 @@ def main():
     sampler.stop_flag = True
     ms = e0.elapsed_time(e1)
     st = sim.stats()
-    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    ntot = torch.tensor([float(n)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        dist.all_reduce(ntot, op=dist.ReduceOp.SUM)
-    ms_all, n_all = float(tmax.item()), float(ntot.item())
+    ms_all, n_all = reduce_over_ranks(ms, n, world, "cuda")
     value = n_all * args.steps / (ms_all * 1e-3)
 
     # ---- end-to-end through the C ABI with HOST buffers: upload state, step, download results, every step
@@ -224,10 +236,11 @@ def main():
         per_stage = {k[3:]: st[k] / K for k in st if k.startswith("ms_") and k != "ms_total"}
         flops = {"density": pairs * (FLOP_PER_PAIR_DENSITY_GATHER + FLOP_PER_PAIR_DENSITY_SWEEP * sweeps),
                  "forces": pairs * FLOP_PER_PAIR_FORCE,
-                 "traverse": pairs * FLOP_PER_PAIR_TEST * 2}
+                 "traverse": pairs * FLOP_PER_PAIR_TEST}
         bytes_ = {"keys": 36 * n, "sort": 200 * n, "permute": 216 * n, "tree": 60 * n, "aabb": 148 * n,
                   "scan": 12 * n, "leapfrog": 272 * n}
         kernels = {}
+        per_stage = {k: v for k, v in per_stage.items() if v > 0.0}
         for k, v in per_stage.items():
             if k in flops:
                 ach = flops[k] / (v * 1e-3) * 1e-12
@@ -237,7 +250,8 @@ def main():
                 kernels[k] = {"ms": v, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
         dom = max(per_stage, key=per_stage.get)
         roofline = dict(kernels[dom])
-        roofline.update({"kernel": dom, "traffic": None,
+        traffic = NCU_TRAFFIC_BYTES_CUBE256.get(dom) if args.workload == "cube256" else None
+        roofline.update({"kernel": dom, "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
                          "peak_source": "sph_measure_fp64_peak DFMA microbenchmark, this run" if dom in flops else hbm_src,
                          "share_of_step": per_stage[dom] / sum(per_stage.values())})
         cpu = None

@@ -275,3 +275,96 @@ def test_neighbour_cache_build_only(make):
     st = sim.stats()
     assert st["nbr_min"] == np.diff(oo).min() and st["nbr_max"] == np.diff(oo).max()
     sim.close()
+
+
+def test_nonuniform_masses():
+    """Unequal particle masses select the density kernel variant that keeps per-neighbour masses (the equal-mass
+    variant factors the mass out of the sums); both must agree with the oracle."""
+    w = W.random_cloud(4000, seed=11, periodic=True, clustered=False)
+    w.mass = w.mass * (0.5 + W.splitmix_u01(77, np.arange(w.n, dtype=np.uint64), 0))
+    w.h0 = 1.2 * (w.mass / w.mass.sum()) ** (1.0 / 3.0)
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    sim.step_leapfrog()
+    sim.close()
+
+
+def _sampled_parity(w, sim, centre, half):
+    """Full-size parity on a sample: targets = particles within `half` (per axis, periodic distance) of `centre`;
+    the oracle evaluates them on the 2-hop closure (targets' neighbours need rho, Omega, hence their own complete
+    neighbour lists), with the plain definitions, from the same h^n = h0. Needs a white step without chi-restart."""
+    box, p = O.workload_box_params(w)
+    assert sim.stats()["restarts"] == 0
+    f = {k: v.numpy() for k, v in sim.get_fields(("h", "rho", "omega", "acc", "dudt"), host=True).items()}
+    L = np.array(w.box_hi) - np.array(w.box_lo)
+    hmax = max(float(w.h0.max()), float(f["h"].max()))
+    rc = 2.0 * p.chi * hmax
+    d = np.abs(w.pos - np.asarray(centre, dtype=np.float64)[:, None])
+    for k in range(3):
+        if w.periodic[k]:
+            d[k] = np.minimum(d[k], L[k] - d[k])
+    dm = d.max(axis=0)
+    sub = np.nonzero(dm <= half + 2.02 * rc)[0]
+    tgt = np.nonzero(dm[sub] <= half)[0]
+    assert tgt.size > 500 and sub.size < 400_000
+    ps, vs = np.ascontiguousarray(w.pos[:, sub]), np.ascontiguousarray(w.vel[:, sub])
+    ms, us, hs = w.mass[sub].copy(), w.u[sub].copy(), w.h0[sub].copy()
+    oo, oi = O.neighbours(ps, hs, box, p.chi, "grid")
+    dn = O.density(ps, ms, hs, oo, oi, box, p)
+    hop1 = np.unique(oi[np.concatenate([np.arange(oo[t], oo[t + 1]) for t in tgt]).astype(np.int64)])
+    assert not dn["exceeded"][hop1].any()
+    acc, dudt, _ = O.forces(ps, vs, ms, dn["h"], dn["rho"], dn["omega"], us, oo, oi, box, p)
+    g = sub[tgt]
+    assert np.max(np.abs(f["h"][g] / dn["h"][tgt] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["rho"][g] / dn["rho"][tgt] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["omega"][g] - dn["omega"][tgt])) < 1e-9
+    cs2 = p.gamma * (p.gamma - 1.0) * np.abs(w.u).max()
+    amax = max(np.abs(f["acc"]).max(), 1e-3 * cs2 / hmax)          # global max |a| (north_star), floored as above
+    dmax = max(np.abs(f["dudt"]).max(), 1e-3 * cs2 ** 1.5 / hmax)
+    assert np.max(np.abs(f["acc"][:, g] - acc[:, tgt])) <= TOL_ACC * amax
+    assert np.max(np.abs(f["dudt"][g] - dudt[tgt])) <= TOL_ACC * dmax
+    # neighbour counts of the targets (sorted-slot order -> original ids through the permutation)
+    _, perm = sim.get_keys_perm()
+    offs = np.empty(w.n + 1, dtype=np.uint64)
+    from paper_2503_09713_b200 import binding as B
+    sim._check(sim.lib.sph_get_neighbours(sim.ctx, B.SPH_MEM_HOST, B._ptr(offs), None, 0))
+    cnt_orig = np.empty(w.n, dtype=np.int64)
+    cnt_orig[perm] = np.diff(offs).astype(np.int64)
+    assert np.array_equal(cnt_orig[g], np.diff(oo).astype(np.int64)[tgt])
+    return tgt.size
+
+
+def _invariants(w, sim):
+    """Properties that hold at any size: sorted keys, valid permutation, sum m a = 0 (periodic, no external force)."""
+    keys, perm = sim.get_keys_perm()
+    assert np.all(keys[1:] >= keys[:-1])
+    assert np.array_equal(np.sort(perm), np.arange(w.n, dtype=perm.dtype))
+    f = {k: v.numpy() for k, v in sim.get_fields(("acc",), host=True).items()}
+    ma = (w.mass * f["acc"]).sum(axis=1)
+    assert np.all(np.abs(ma) < 1e-10 * np.abs(w.mass * f["acc"]).sum(axis=1).max() + 1e-300)
+
+
+def test_c2_full_size_sampled_parity():
+    """BASELINE config 2 at full size (256^3 = 16.8 M particles), the workload and launch configuration bench.py
+    times: invariants on everything, oracle parity on two sampled regions (interior; across the periodic corner)."""
+    w = W.cube(256, jitter=0.1, steps=5)
+    sim = _sim(w)
+    _invariants(w, sim)
+    n1 = _sampled_parity(w, sim, (0.43, 0.52, 0.37), 0.02)
+    n2 = _sampled_parity(w, sim, (0.0, 1.0, 0.0), 0.02)          # wraps around all three periodic faces
+    assert n1 > 900 and n2 > 900
+    st = sim.stats()
+    assert st["n_groups"] == w.n // 32 and 75 < st["nbr_mean"] < 90
+    sim.step_leapfrog()                                           # and one full step in that configuration
+    assert sim.stats()["steps"] == 1
+    sim.close()
+
+
+def test_c1_sod_full_size_sampled_parity():
+    """BASELINE config 1 at full size (589,824 particles): sampled parity across the density jump at x = 0."""
+    w = W.config(1)
+    sim = _sim(w)
+    _invariants(w, sim)
+    _sampled_parity(w, sim, (0.0, 0.0, 0.0), 0.03)
+    _sampled_parity(w, sim, (0.5, 0.125, -0.125), 0.03)          # the periodic seam, a box corner
+    sim.close()
