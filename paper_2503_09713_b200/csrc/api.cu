@@ -2,6 +2,7 @@
 // getters/setters and per-stage CUDA-event timers. All arithmetic of the hot path lives in the kernels of the
 // sibling .cu files; there is no CPU fallback anywhere in this library.
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -138,6 +139,9 @@ static int cache_build(sph_ctx* c) {
         if (s.n_cand_overflow)
             return fail(c, SPH_ERR_CAP, "%u leaf groups have more than 65535 candidates (16-bit local index)",
                         s.n_cand_overflow);
+        if (getenv("SPH_DEBUG"))
+            fprintf(stderr, "[sph] groups %u nc_max %u nb_max %u fallback %u nbr_min %u nbr_max %u lists %llu buckets %llu\n",
+                    s.n_groups, s.nc_max, s.nb_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.bkt_cursor);
         c->n_groups = s.n_groups;
         c->nc_max = s.nc_max;
         c->n_neigh = s.n_neigh;
