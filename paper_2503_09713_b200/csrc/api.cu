@@ -140,8 +140,8 @@ static int cache_build(sph_ctx* c) {
             return fail(c, SPH_ERR_CAP, "%u leaf groups have more than 65535 candidates (16-bit local index)",
                         s.n_cand_overflow);
         if (getenv("SPH_DEBUG"))
-            fprintf(stderr, "[sph] groups %u nc_max %u nb_max %u fallback %u nbr_min %u nbr_max %u lists %llu buckets %llu\n",
-                    s.n_groups, s.nc_max, s.nb_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.bkt_cursor);
+            fprintf(stderr, "[sph] groups %u nc_max %u fallback %u nbr_min %u nbr_max %u lists %llu candidates %llu\n",
+                    s.n_groups, s.nc_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.cslot_cursor);
         c->n_groups = s.n_groups;
         c->nc_max = s.nc_max;
         c->n_neigh = s.n_neigh;
@@ -150,8 +150,8 @@ static int cache_build(sph_ctx* c) {
             SPH_TRY(grow_pool(c, &c->lists, &c->list_cap, s.list_cursor + s.list_cursor / 8 + 4096));
             redo = true;
         }
-        if (s.bkt_cursor > c->bkt_cap) {
-            SPH_TRY(grow_pool(c, &c->bkt, &c->bkt_cap, s.bkt_cursor + s.bkt_cursor / 8 + 1024));
+        if (s.cslot_cursor > c->cslot_cap) {
+            SPH_TRY(grow_pool(c, &c->cslot, &c->cslot_cap, s.cslot_cursor + s.cslot_cursor / 8 + 4096));
             redo = true;
         }
         if ((uint64_t)s.n_groups > c->ginfo_cap) {
@@ -238,6 +238,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->visit, n));
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
     SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
+    SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
     // cache pools start empty: the first traversal only counts, then they are sized from its totals
     c->scan_tiles = scan_scratch_tiles(N);
     SPH_TRY(dalloc(c, &c->scan_status, (size_t)c->scan_tiles));

@@ -36,10 +36,9 @@ struct __align__(16) NodeRec {
 };
 static_assert(sizeof(NodeRec) == 64, "NodeRec must be 64 bytes");
 
-// One bucket of a group's candidate array: sorted slots [lo, lo + n) hold local candidates [cstart, cstart + n),
-// n = next entry's cstart - cstart (the table ends with a sentinel whose cstart is the group's candidate count).
-struct BucketRec { uint32_t lo, cstart; };
-struct __align__(16) GroupRec { uint32_t bkt_off_lo, bkt_off_hi, nb, nc; };
+// One leaf group's entry in the neighbour cache: where its candidate array (sorted-slot indices, u32) starts in the
+// candidate pool and how many candidates it has (bit 31 of nc: some candidate may wrap around a periodic axis).
+struct __align__(16) GroupRec { uint32_t cs_off_lo, cs_off_hi, nc, pad; };
 
 enum Stage { ST_KEYS = 0, ST_SORT, ST_PERMUTE, ST_TREE, ST_AABB, ST_TRAVERSE, ST_SCAN, ST_DENSITY, ST_FORCES,
              ST_LEAPFROG, ST_COUNT };
@@ -61,9 +60,8 @@ struct DevScalars {
     double t;                        // simulated time (sum of the dt actually used)
     // neighbour-cache allocation state of the last traversal (bump allocators + limits seen)
     unsigned long long list_cursor;  // 16-bit list entries handed out (each group's block padded to 8 entries)
-    unsigned long long bkt_cursor;   // bucket-table entries handed out (nb + 1 per group)
+    unsigned long long cslot_cursor; // candidate-pool entries handed out (each group's array padded to 4)
     unsigned int nc_max;             // largest candidate count of any group
-    unsigned int nb_max;             // largest bucket count of any group
     unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
@@ -102,14 +100,15 @@ struct sph_ctx {
     uint32_t* gscan = nullptr;          // N+1 exclusive scan of gflag (u32)
     uint32_t* grp_lo = nullptr;         // Ng+1 first slot of group g (grp_lo[Ng] = N)
     int64_t n_groups = 0;
-    // neighbour cache, group-local (a4): per group a bucket table (slot ranges = the group's
-    // candidate array) and per particle an ascending list of 16-bit indices into that candidate array
+    // neighbour cache, group-local (a4): per group a candidate array (sorted slots of the particles
+    // that passed the traversal's prefilter) and per particle an ascending list of 16-bit indices into it
     uint32_t* cnt = nullptr;            // N+1  list length of each sorted slot
     uint64_t* lstart = nullptr;         // N    first entry of each slot's list in `lists`
     uint16_t* lists = nullptr;
     uint64_t list_cap = 0;
-    sph::BucketRec* bkt = nullptr;      // bucket tables, nb + 1 entries per group (last = sentinel holding nc)
-    uint64_t bkt_cap = 0;
+    uint32_t* cslot = nullptr;          // candidate pool
+    uint64_t cslot_cap = 0;
+    uint32_t* trav_scratch = nullptr;   // per-warp candidate rows of the traversal grid
     sph::GroupRec* ginfo = nullptr;     // one per group
     uint64_t ginfo_cap = 0;
     uint32_t nc_max = 0;
@@ -163,7 +162,8 @@ int launch_permute(sph_ctx* c);                                // permute.cu
 int launch_tree(sph_ctx* c);                                   // tree.cu   karras + groups
 int launch_aabb(sph_ctx* c);                                   // tree.cu
 int launch_traverse(sph_ctx* c);                               // neigh.cu  single pass: walk, test, write cache
-int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out);        // neigh.cu  group-local lists -> global CSR (getter)
+int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out);
+size_t trav_scratch_entries();                                  // neigh.cu  u32 entries of the traversal's scratch rows        // neigh.cu  group-local lists -> global CSR (getter)
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
 int launch_density(sph_ctx* c);                                // density.cu

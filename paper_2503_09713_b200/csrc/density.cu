@@ -143,7 +143,7 @@ template <bool UNIM>
 __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
-    const GroupRec* __restrict__ ginfo, const BucketRec* __restrict__ bkt, const uint32_t* __restrict__ cnt,
+    const GroupRec* __restrict__ ginfo, const uint32_t* __restrict__ cslot, const uint32_t* __restrict__ cnt,
     const uint64_t* __restrict__ lstart, const uint16_t* __restrict__ lists, DensBox db, DensPar dp, uint32_t ncap,
     double* __restrict__ hout, double* __restrict__ rho, double* __restrict__ omega, DevScalars* sc) {
     extern __shared__ __align__(16) double dsm[];
@@ -156,7 +156,8 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const uint32_t g = blockIdx.x;
     const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
     const GroupRec gr = ginfo[g];
-    const BucketRec* tab = bkt + (((uint64_t)gr.bkt_off_hi << 32) | gr.bkt_off_lo);
+    const uint32_t* cs = cslot + (((uint64_t)gr.cs_off_hi << 32) | gr.cs_off_lo);
+    const uint32_t nc = gr.nc & 0x7fffffffu;
     const bool gwrap = (gr.nc >> 31) != 0u;
 
     // this octet's particle (loads issued before the staging loop so that their latency overlaps it)
@@ -167,14 +168,10 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const uint16_t* li = lists + lstart[a];
     const int n = pv ? (int)cnt[a] : 0;
 
-    // ---- stage the candidate array: one bucket (<= 32 consecutive slots) per warp iteration ----
-    for (uint32_t j = warp; j < gr.nb; j += kDensWarps) {
-        const BucketRec b0 = tab[j];
-        const uint32_t bn = tab[j + 1].cstart - b0.cstart;
-        if (lane < bn) {
-            const uint32_t s = b0.lo + lane, c = b0.cstart + lane;
-            cp_async8(sx + c, x + s); cp_async8(sy + c, y + s); cp_async8(sz + c, z + s); cp_async8(sm + c, m + s);
-        }
+    // ---- stage the candidate array (slots are mostly runs of consecutive indices: coalesced sectors) ----
+    for (uint32_t c = threadIdx.x; c < nc; c += kDensWarps * 32) {
+        const uint32_t s = cs[c];
+        cp_async8(sx + c, x + s); cp_async8(sy + c, y + s); cp_async8(sz + c, z + s); cp_async8(sm + c, m + s);
     }
     // the first 96 list entries of the octet's particle (two 16-bit indices per register), in flight together with
     // the staging copies
@@ -235,11 +232,11 @@ int launch_density(sph_ctx* c) {
     // all masses equal (checked once at init): the kernel variant without per-neighbour mass registers
     if (c->uniform_mass)
         k_density<true><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->bkt, c->cnt, c->lstart, c->lists, db,
+            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db,
             dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
     else
         k_density<false><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->bkt, c->cnt, c->lstart, c->lists, db,
+            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db,
             dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
     c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());

@@ -14,12 +14,13 @@
 //     by a positive constant and squaring are monotone, so max() commutes with them exactly. Buckets whose union
 //     box with the group spans at most L/2 on every periodic axis cannot wrap and take a loop without the
 //     minimum-image selects (the decision is exact).
-//   Output (the cache): the group's bucket table (its candidate array = concatenated slot ranges)
-//     and, per particle, the ascending list of 16-bit indices into that candidate array. Hits are buffered in
-//     shared memory and written out coalesced once the group is complete; space comes from two bump allocators
-//     (count -> allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed).
-//     A group whose buffers overflow (a list longer than kHitCap, more than kBktCap buckets) allocates from its
-//     exact counts and walks a second time writing directly.
+//   Output (the cache): the group's candidate array (the sorted slots of the candidates that passed
+//     the prefilter, in traversal order) and, per particle, the ascending list of 16-bit indices into that
+//     candidate array. Hits are buffered in shared memory, candidate slots in a per-warp global scratch row, and
+//     both are written out coalesced once the group is complete; space comes from two bump allocators (count ->
+//     allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed). A group whose
+//     buffers overflow (a list longer than kHitCap, more than kScrCap candidates) allocates from its exact
+//     counts and walks a second time writing directly.
 #include "common.cuh"
 
 namespace sph {
@@ -31,7 +32,7 @@ constexpr int kPendCap = 64;             // candidate buckets buffered before st
 constexpr int kHitCap = 112;             // buffered hits per lane
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
 constexpr int kHitStride = kHitCap + kHitSlack + 2;   // in u16: 73 words per lane row (odd: rows start in distinct banks)
-constexpr int kBktCap = 126;             // buffered bucket records per group
+constexpr int kScrCap = 2048;            // candidate slots buffered per group (global scratch row of the warp)
 constexpr uint32_t kLeafBit = 0x80000000u;
 constexpr uint32_t kWrapBit = 0x80000000u;
 
@@ -46,7 +47,6 @@ struct TravWarpSmem {
     uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
     double2 cxy[32], czr[32];                 // staged candidates (compacted): {x, y}, {z, (R_kern chi h)^2}
     uint32_t cid[32];                         // their indices in the group's candidate array
-    BucketRec gb[kBktCap + 2];
     uint16_t hits[32 * kHitStride];
 };
 
@@ -55,8 +55,9 @@ struct TravOut {
     uint64_t* lstart;
     uint16_t* lists;
     uint64_t list_cap;
-    BucketRec* bkt;
-    uint64_t bkt_cap;
+    uint32_t* cslot;
+    uint64_t cslot_cap;
+    uint32_t* scratch;       // kScrCap entries per warp of the grid
     GroupRec* ginfo;
     uint64_t ginfo_cap;
 };
@@ -86,9 +87,9 @@ struct GroupCtx {
     double rc2g;          // (R_kern chi hmax_group)^2, for the per-candidate prefilter
     uint32_t nhit;        // per lane: hits so far (exact)
     uint32_t wpos;        // per lane, buffered mode: store position in the lane's row (clamped to kHitCap per bucket)
-    uint32_t nbk, nc;     // warp-uniform: buckets and candidates so far
+    uint32_t ncs;         // warp-uniform: candidates (prefilter survivors) so far
     uint16_t* lptr;       // DIRECT: this lane's list in global memory
-    BucketRec* bptr;      // DIRECT: the group's bucket table in global memory
+    uint32_t* cptr;       // candidate slots: the warp's scratch row, or (DIRECT) the group's array in global memory
     bool can_write;       // DIRECT: allocation succeeded
     bool anywrap;         // warp-uniform: some bucket of this group may wrap around a periodic axis
 };
@@ -154,18 +155,13 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
         if (keep) {
             s.cxy[pos] = make_double2(cx, cy);
             s.czr[pos] = make_double2(cz, rc2);
-            s.cid[pos] = G.nc + lane;                   // index in the group's candidate array
+            s.cid[pos] = G.ncs + pos;                   // index in the group's candidate array
+            if (DIRECT ? G.can_write : (G.ncs + pos < (uint32_t)kScrCap)) G.cptr[G.ncs + pos] = blo + lane;
         }
         if (lane < 4u && nk + lane < nk4) {             // pad to a multiple of four with candidates nobody can hit
             s.cxy[nk + lane] = make_double2(1e300, 1e300);
             s.czr[nk + lane] = make_double2(1e300, 0.0);
             s.cid[nk + lane] = 0u;
-        }
-        if (lane == 0) {
-            BucketRec r;
-            r.lo = blo; r.cstart = G.nc;
-            if (DIRECT) { if (G.can_write) G.bptr[G.nbk] = r; }
-            else if (G.nbk < (uint32_t)kBktCap) s.gb[G.nbk] = r;
         }
         __syncwarp();
         const uint32_t w0 = (uint32_t)__cvta_generic_to_shared(&s.hits[row + G.wpos]);
@@ -198,8 +194,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             G.wpos += got;
             if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;   // overflowed row: keep counting, stop growing
         }
-        G.nc += bn;
-        G.nbk += 1u;
+        G.ncs += nk;
     }
 }
 
@@ -209,7 +204,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.nbk = 0u; G.nc = 0u; G.anywrap = false;
+    G.nhit = 0u; G.wpos = 0u; G.ncs = 0u; G.anywrap = false;
     int sp = 1, nb = 0;
     __syncwarp();
     if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
@@ -296,7 +291,8 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
     const unsigned lane = lane_id();
     const unsigned lt = lanemask_lt();
     const uint32_t n_groups = sc->n_groups;
-    unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u, nbmax = 0u;
+    unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u;
+    uint32_t* const scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
 
     for (;;) {
         uint32_t g = 0;
@@ -321,13 +317,13 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
             G.rc2g = __dmul_rn(rcg, rcg);
         }
         if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
-        G.lptr = nullptr; G.bptr = nullptr; G.can_write = false;
+        G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
 
         walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
-        // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and bucket table ----
+        // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and candidate slots ----
         const uint32_t nhit = qv ? G.nhit : 0u;
-        const uint32_t nbk = G.nbk, nc = G.nc;
+        const uint32_t nc = G.ncs, nc4 = (nc + 3u) & ~3u;
         uint32_t incl = nhit;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -339,12 +335,12 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         unsigned long long lbase = 0, bbase = 0;
         if (lane == 0) {
             lbase = atomicAdd(&sc->list_cursor, (unsigned long long)((total + 7u) & ~7u));
-            bbase = atomicAdd(&sc->bkt_cursor, (unsigned long long)(nbk + 1u));
+            bbase = atomicAdd(&sc->cslot_cursor, (unsigned long long)nc4);
             atomicAdd(&sc->n_neigh, (unsigned long long)total);
         }
         lbase = __shfl_sync(0xffffffffu, lbase, 0);
         bbase = __shfl_sync(0xffffffffu, bbase, 0);
-        const bool fits = (lbase + ((total + 7u) & ~7u) <= out.list_cap) && (bbase + nbk + 1u <= out.bkt_cap) &&
+        const bool fits = (lbase + ((total + 7u) & ~7u) <= out.list_cap) && (bbase + nc4 <= out.cslot_cap) &&
                           ((uint64_t)g < out.ginfo_cap) && (nc <= 65535u);
         const uint64_t my_start = lbase + (incl - nhit);
         if (qv) {
@@ -354,15 +350,14 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         if (fits) {
             if (lane == 0) {
                 GroupRec r;
-                r.bkt_off_lo = (uint32_t)(bbase & 0xffffffffull); r.bkt_off_hi = (uint32_t)(bbase >> 32);
-                r.nb = nbk; r.nc = nc | (G.anywrap ? 0x80000000u : 0u);
+                r.cs_off_lo = (uint32_t)(bbase & 0xffffffffull); r.cs_off_hi = (uint32_t)(bbase >> 32);
+                r.nc = nc | (G.anywrap ? 0x80000000u : 0u); r.pad = 0u;
                 out.ginfo[g] = r;
-                BucketRec sentinel; sentinel.lo = 0u; sentinel.cstart = nc;
-                out.bkt[bbase + nbk] = sentinel;
             }
-            const bool overflow = (maxhit > (uint32_t)kHitCap) || (nbk > (uint32_t)kBktCap);
+            const bool overflow = (maxhit > (uint32_t)kHitCap) || (nc > (uint32_t)kScrCap);
             if (!overflow) {
-                for (uint32_t j = lane; j < nbk; j += 32) out.bkt[bbase + j] = s.gb[j];
+                __syncwarp();
+                for (uint32_t j = lane; j < nc; j += 32) out.cslot[bbase + j] = scr_row[j];
                 // lists: the warp copies one particle's buffered list at a time (coalesced 16-bit stores)
                 for (uint32_t p = 0; p < nq; ++p) {
                     const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
@@ -372,7 +367,7 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
             } else {
                 // fallback: second walk writing directly at the now-known positions
                 G.lptr = out.lists + my_start;
-                G.bptr = out.bkt + bbase;
+                G.cptr = out.cslot + bbase;
                 G.can_write = true;
                 walk<true>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
                 if (lane == 0) atomicAdd(&sc->n_fallback, 1u);
@@ -381,7 +376,6 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         if (nc > 65535u && lane == 0) atomicAdd(&sc->n_cand_overflow, 1u);
         if (qv) { mn = min(mn, nhit); mx = max(mx, nhit); }
         ncmax = max(ncmax, nc);
-        nbmax = max(nbmax, nbk);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -391,16 +385,18 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
     if (lane == 0) {
         if (mx >= mn) { atomicMin(&sc->nbr_min, mn); atomicMax(&sc->nbr_max, mx); }
         atomicMax(&sc->nc_max, ncmax);
-        atomicMax(&sc->nb_max, nbmax);
     }
 }
 
 __global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc) {
     *work_counter = 0u;
     sc->nbr_min = 0xffffffffu; sc->nbr_max = 0u;
-    sc->list_cursor = 0ull; sc->bkt_cursor = 0ull; sc->n_neigh = 0ull;
-    sc->nc_max = 0u; sc->nb_max = 0u; sc->n_cand_overflow = 0u; sc->n_fallback = 0u;
+    sc->list_cursor = 0ull; sc->cslot_cursor = 0ull; sc->n_neigh = 0ull;
+    sc->nc_max = 0u; sc->n_cand_overflow = 0u; sc->n_fallback = 0u;
 }
+
+constexpr int kTravBlocks = 148 * 2;     // persistent grid: two CTAs per SM (shared-memory bound)
+size_t trav_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * kScrCap; }
 
 int launch_traverse(sph_ctx* c) {
     static bool attr_set = false;
@@ -421,12 +417,12 @@ int launch_traverse(sph_ctx* c) {
     const double rk_chi = kRkern * c->p.chi;
     TravOut out;
     out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
-    out.bkt = c->bkt; out.bkt_cap = c->bkt_cap; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
+    out.cslot = c->cslot; out.cslot_cap = c->cslot_cap; out.scratch = c->trav_scratch; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
     uint32_t* wc = c->sort_counters + 8;   // spare counter word
     k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc);
     // persistent grid: two CTAs per SM (shared-memory bound), work handed out through an atomic counter
     const int64_t warps_needed = (c->N + 31) / 32;
-    unsigned blocks = (unsigned)min((int64_t)148 * 2, (warps_needed + kTravWarps - 1) / kTravWarps);
+    unsigned blocks = (unsigned)min((int64_t)kTravBlocks, (warps_needed + kTravWarps - 1) / kTravWarps);
     if (blocks == 0) blocks = 1;
     k_traverse<<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
                                                              c->grp_lo, tb, rk_chi, out, wc, c->d_sc);
@@ -438,7 +434,7 @@ int launch_traverse(sph_ctx* c) {
 // ---- getter path: group-local lists -> global CSR over sorted slots (sph_get_neighbours) ----
 __global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t* __restrict__ gscan,
                                                       const GroupRec* __restrict__ ginfo,
-                                                      const BucketRec* __restrict__ bkt,
+                                                      const uint32_t* __restrict__ cslot,
                                                       const uint32_t* __restrict__ cnt,
                                                       const uint64_t* __restrict__ lstart,
                                                       const uint16_t* __restrict__ lists,
@@ -447,20 +443,15 @@ __global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t*
     if (a >= N) return;
     const uint32_t g = gscan[a + 1] - 1u;          // gscan = exclusive scan of the group-start flags
     const GroupRec gr = ginfo[g];
-    const BucketRec* tab = bkt + (((uint64_t)gr.bkt_off_hi << 32) | gr.bkt_off_lo);
+    const uint32_t* cs = cslot + (((uint64_t)gr.cs_off_hi << 32) | gr.cs_off_lo);
     const uint16_t* li = lists + lstart[a];
     const uint32_t n = cnt[a];
-    uint32_t j = 0;
-    uint64_t o = offs[a];
-    for (uint32_t k = 0; k < n; ++k) {
-        const uint32_t cl = li[k];
-        while (tab[j + 1].cstart <= cl) ++j;       // lists ascend, so the bucket pointer only moves forward
-        idx[o + k] = tab[j].lo + (cl - tab[j].cstart);
-    }
+    const uint64_t o = offs[a];
+    for (uint32_t k = 0; k < n; ++k) idx[o + k] = cs[li[k]];
 }
 
 int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out) {
-    k_cache_to_csr<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->bkt, c->cnt, c->lstart,
+    k_cache_to_csr<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->cslot, c->cnt, c->lstart,
                                                              c->lists, c->offs, idx_out);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
