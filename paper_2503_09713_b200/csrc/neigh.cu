@@ -62,12 +62,17 @@ struct TravOut {
     uint64_t ginfo_cap;
 };
 
+// min / max by compare-and-select: operands here are never NaN, and fmin()/fmax() expand to a NaN-safe sequence of
+// about six instructions on sm_100
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+
 // separation of two intervals [alo,ahi], [blo,bhi] along one axis (0 if they overlap), minimum over periodic images
 __device__ __forceinline__ double axis_gap(double alo, double ahi, double blo, double bhi, double L, int periodic) {
-    double g = fmax(fmax(blo - ahi, alo - bhi), 0.0);
+    double g = dmax(dmax(blo - ahi, alo - bhi), 0.0);
     if (periodic) {
-        g = fmin(g, fmax(blo + L - ahi, 0.0));
-        g = fmin(g, fmax(alo - bhi + L, 0.0));
+        g = dmin(g, dmax(blo + L - ahi, 0.0));
+        g = dmin(g, dmax(alo - bhi + L, 0.0));
     }
     return g;
 }
@@ -144,10 +149,10 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
         // Buckets that may wrap keep every candidate.
         bool keep = lane < bn;
         if (keep && !wrap) {
-            const double gx = fmax(fmax(G.gxl - cx, cx - G.gxh), 0.0);
-            const double gy = fmax(fmax(G.gyl - cy, cy - G.gyh), 0.0);
-            const double gz = fmax(fmax(G.gzl - cz, cz - G.gzh), 0.0);
-            keep = gx * gx + gy * gy + gz * gz <= fmax(rc2, G.rc2g) * (1.0 + 1e-9);
+            const double gx = dmax(dmax(G.gxl - cx, cx - G.gxh), 0.0);
+            const double gy = dmax(dmax(G.gyl - cy, cy - G.gyh), 0.0);
+            const double gz = dmax(dmax(G.gzl - cz, cz - G.gzh), 0.0);
+            keep = gx * gx + gy * gy + gz * gz <= dmax(rc2, G.rc2g) * (1.0 + 1e-9);
         }
         const unsigned km = __ballot_sync(0xffffffffu, keep);
         const uint32_t nk = (uint32_t)__popc(km), nk4 = (nk + 3u) & ~3u, pos = (uint32_t)__popc(km & lt);
@@ -238,15 +243,15 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                 small = (rhi - rlo + 1) <= (uint32_t)kGroup;
             }
             // group-group criterion, conservative under rounding (tiny pad)
-            const double ext = rk_chi * fmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
+            const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
             const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
             const double ggy = axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]);
             const double ggz = axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]);
             pass = ggx * ggx + ggy * ggy + ggz * ggz <= ext * ext;
             // can any (query, candidate) separation exceed L/2 on a periodic axis? (exact: rounding is monotone)
-            wrap = (tb.periodic[0] && (fmax(G.gxh, bhi[0]) - fmin(G.gxl, blo[0]) > tb.halfL[0])) ||
-                   (tb.periodic[1] && (fmax(G.gyh, bhi[1]) - fmin(G.gyl, blo[1]) > tb.halfL[1])) ||
-                   (tb.periodic[2] && (fmax(G.gzh, bhi[2]) - fmin(G.gzl, blo[2]) > tb.halfL[2]));
+            wrap = (tb.periodic[0] && (dmax(G.gxh, bhi[0]) - dmin(G.gxl, blo[0]) > tb.halfL[0])) ||
+                   (tb.periodic[1] && (dmax(G.gyh, bhi[1]) - dmin(G.gyl, blo[1]) > tb.halfL[1])) ||
+                   (tb.periodic[2] && (dmax(G.gzh, bhi[2]) - dmin(G.gzl, blo[2]) > tb.halfL[2]));
         }
         const bool push = pass && !small, emit = pass && small;
         const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
