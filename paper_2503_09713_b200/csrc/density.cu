@@ -145,6 +145,7 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
     const GroupRec* __restrict__ ginfo, const uint32_t* __restrict__ cslot, const uint32_t* __restrict__ cnt,
     const uint64_t* __restrict__ lstart, const uint16_t* __restrict__ lists, DensBox db, DensPar dp, uint32_t ncap,
+    uint32_t nc_lo, uint32_t nc_hi,
     double* __restrict__ hout, double* __restrict__ rho, double* __restrict__ omega, DevScalars* sc) {
     extern __shared__ __align__(16) double dsm[];
     double* sx = dsm;
@@ -158,6 +159,7 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const GroupRec gr = ginfo[g];
     const uint32_t* cs = cslot + (((uint64_t)gr.cs_off_hi << 32) | gr.cs_off_lo);
     const uint32_t nc = gr.nc & 0x7fffffffu;
+    if (nc <= nc_lo || nc > nc_hi) return;       // this launch serves the groups with nc in (nc_lo, nc_hi]
     const bool gwrap = (gr.nc >> 31) != 0u;
 
     // this octet's particle (loads issued before the staging loop so that their latency overlaps it)
@@ -223,22 +225,32 @@ int launch_density(sph_ctx* c) {
     }
     DensPar dp;
     dp.hfact = c->p.hfact; dp.chi = c->p.chi; dp.lambda = c->p.lambda; dp.eps_h = c->p.eps_h; dp.max_iter = c->p.max_h_iter;
-    const uint32_t ncap = (c->nc_max + 31u) & ~31u;
-    const size_t smem = (size_t)ncap * 4 * sizeof(double);
-    if (smem > 227 * 1024)
+    if ((size_t)c->nc_max * 4 * sizeof(double) > 227 * 1024)
         return fail(c, SPH_ERR_CAP, "a leaf group has %u candidates: more than the density kernel can stage (%d)",
                     c->nc_max, 227 * 1024 / 32);
     k_density_reset<<<1, 1, 0, c->stream>>>(c->d_sc);
-    // all masses equal (checked once at init): the kernel variant without per-neighbour mass registers
-    if (c->uniform_mass)
-        k_density<true><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db,
-            dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
-    else
-        k_density<false><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-            c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db,
-            dp, ncap, c->hnew, c->rho, c->omega, c->d_sc);
-    c->launches += 2;
+    c->launches++;
+    // The staged candidate array sizes the CTA's shared memory, hence the occupancy: groups are served in two size
+    // classes (a CTA whose group belongs to the other class exits at once), so that a few crowded groups (density
+    // jumps, disc mid-plane) do not cost everyone else their occupancy. One launch when all groups are small.
+    const uint32_t kSmall = 768;
+    for (int cls = 0; cls < 2; ++cls) {
+        const uint32_t lo = cls == 0 ? 0u : kSmall, hi = cls == 0 ? kSmall : 0x7fffffffu;
+        if (cls == 1 && c->nc_max <= kSmall) break;
+        // nc = 0 cannot occur (a particle is its own neighbour); lo = 0 therefore excludes nothing in class 0
+        const uint32_t ncap = ((cls == 0 ? (c->nc_max < kSmall ? c->nc_max : kSmall) : c->nc_max) + 31u) & ~31u;
+        const size_t smem = (size_t)ncap * 4 * sizeof(double);
+        // all masses equal (checked once at init): the kernel variant without per-neighbour mass registers
+        if (c->uniform_mass)
+            k_density<true><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+                c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists,
+                db, dp, ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
+        else
+            k_density<false><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+                c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists,
+                db, dp, ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
+        c->launches++;
+    }
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }

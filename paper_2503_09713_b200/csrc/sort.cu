@@ -75,7 +75,7 @@ struct SortSmem {
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(kSortThreads) k_onesweep(const uint64_t* __restrict__ kin,
+__global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __restrict__ kin,
                                                             const uint32_t* __restrict__ vin,
                                                             uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                             int64_t N, int shift, const uint32_t* __restrict__ gbase,
@@ -101,17 +101,22 @@ __global__ void __launch_bounds__(kSortThreads) k_onesweep(const uint64_t* __res
         k[i] = (idx < N) ? kin[idx] : ~0ull;
     }
     const unsigned lt = lanemask_lt();
+    // all match masks first (independent MATCH instructions pipeline), then the serial counter updates
+    unsigned mm[kItems];
 #pragma unroll
     for (int i = 0; i < kItems; ++i) {
-        bool valid = (wbase + i * 32) < N;
-        unsigned act = __ballot_sync(0xffffffffu, valid);
-        unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
+        const bool valid = (wbase + i * 32) < N;
+        const unsigned act = __ballot_sync(0xffffffffu, valid);
+        const unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
+        mm[i] = valid ? __match_any_sync(act, d) : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < kItems; ++i) {
+        const bool valid = (wbase + i * 32) < N;
+        const unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
+        const unsigned m = mm[i];
         uint32_t prev = 0;
-        unsigned m = 0;
-        if (valid) {
-            m = __match_any_sync(act, d);
-            prev = s.whist[w][d];
-        }
+        if (valid) prev = s.whist[w][d];
         __syncwarp();
         if (valid && lane == (unsigned)(__ffs(m) - 1)) s.whist[w][d] = prev + __popc(m);
         __syncwarp();
