@@ -68,35 +68,40 @@ def make_workload(name: str, seed_offset: int = 0):
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
-
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """Samples SM clock, power and throttle reasons during the timed region (B200_PROFILING.md recipe) through NVML
+    every 20 ms (nvidia-smi itself takes longer to start than a whole step lasts)."""
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
-        self.index, self.rows, self.stop_flag = index, [], False
+        self.index, self.rows, self.stop_flag, self.max_mhz = index, [], False, None
 
     def run(self):
-        while not self.stop_flag:
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
-                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([x.strip() for x in out.split(",")])
-            except Exception:
-                pass
-            time.sleep(0.2)
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[self.index]) if vis and vis.split(",")[self.index].isdigit() else self.index
+            h = nv.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            while not self.stop_flag:
+                self.rows.append((float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
+                                  nv.nvmlDeviceGetPowerUsage(h) / 1000.0,
+                                  int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))))
+                time.sleep(0.02)
+        except Exception as e:          # no NVML: report that instead of a clock
+            self.err = repr(e)
 
     def summary(self):
         if not self.rows:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
-        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for k, n in enumerate(names) if any(len(r) > 3 + k and r[3 + k].lower().startswith("active") for r in self.rows)]
-        pw = [float(r[2]) for r in self.rows if r[2].replace(".", "").isdigit()]
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(self.rows[0][1]) if self.rows[0][1].replace(".", "").isdigit() else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(self.rows), "reasons": reasons}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable: " + getattr(self, "err", "no samples")]}
+        bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4,
+                "hw_power_brake_slowdown": 0x80}
+        seen = 0
+        for r in self.rows:
+            seen |= r[2]
+        return {"sm_mhz": float(np.median([r[0] for r in self.rows])), "sm_max_mhz": self.max_mhz,
+                "power_w_max": max(r[1] for r in self.rows), "samples": len(self.rows),
+                "reasons": [k for k, b in bits.items() if seen & b]}
 
 
 def oracle_step_rate(n_side: int, steps: int, warmup: int):
@@ -135,19 +140,57 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """BASELINE config 4: the C2 recipe at 64^3 ... 512^3 on one GPU; one JSON line per size with per-kernel times."""
+    import torch
+    from paper_2503_09713_b200 import binding as B, workloads as W
+    torch.cuda.set_device(0)
+    for n_side in (64, 128, 256, 384, 512):
+        w = W.cube(n_side, jitter=0.1, steps=args.steps)
+        try:
+            sim = B.Sim.from_workload(w)
+        except B.SphError as e:
+            print(json.dumps({"sweep_n_side": n_side, "n_particles": w.n, "error": str(e)}))
+            break
+        n = w.n
+        del w
+        for _ in range(max(args.warmup, 1)):
+            sim.step_leapfrog()
+        torch.cuda.synchronize()
+        sim.reset_timers()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            sim.step_leapfrog()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        st = sim.stats()
+        print(json.dumps({"sweep_n_side": n_side, "n_particles": n, "ms_per_step": ms, "value": n / (ms * 1e-3), "unit": UNIT,
+                          "ms_per_kernel": {k[3:]: st[k] / args.steps for k in st if k.startswith("ms_") and k != "ms_total"
+                                            and st[k] > 0},
+                          "neighbours_mean": st["nbr_mean"], "bytes_allocated": st["bytes_allocated"]}), flush=True)
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cube256")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-side", type=int, default=40, help="lattice side of the oracle's bounded sample")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE config 4: sizes 64^3..512^3, one line each")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import torch
     import torch.distributed as dist
