@@ -72,7 +72,11 @@ __global__ void __launch_bounds__(256) k_group_fill(int64_t N, const uint32_t* _
     }
 }
 
-// bottom-up boxes: one thread per leaf; the second thread to reach a node merges its children and goes on
+// bottom-up boxes: one thread per leaf; the second thread to reach a node merges its children and goes on.
+// A node whose two children are both leaves needs no flag: the left leaf's thread merges the pair directly and the
+// right leaf's thread retires at once (about half of all leaves, so half of the bottom-level atomics and fences).
+// Sibling records are read with L2 loads (ld.cg) issued after the flag atomic has returned, so only the release
+// side (record written -> fence -> flag) needs a fence.
 __global__ void __launch_bounds__(256) k_aabb(int64_t N, const double* __restrict__ x, const double* __restrict__ y,
                                               const double* __restrict__ z, const double* __restrict__ h,
                                               NodeRec* nodes, const int32_t* __restrict__ parent, uint32_t* visit) {
@@ -83,15 +87,19 @@ __global__ void __launch_bounds__(256) k_aabb(int64_t N, const double* __restric
     bool cur_leaf = true;
     int32_t node = parent[N - 1 + i];
     while (node >= 0) {
-        __threadfence();                                  // my record (if any) is visible before I announce myself
-        if (atomicAdd(&visit[node], 1u) == 0u) return;    // first arrival: the sibling's thread will carry on
-        __threadfence();
         const int32_t other = nodes[node].other, split = nodes[node].split;
         const int32_t nlo = min(node, other), nhi = max(node, other);
         const bool lleaf = (nlo == split), rleaf = (nhi == split + 1);
         const bool i_am_left = (cur == split) && (cur_leaf == lleaf);
         const int32_t sib = i_am_left ? split + 1 : split;
         const bool sib_leaf = i_am_left ? rleaf : lleaf;
+        if (cur_leaf && sib_leaf) {
+            if (!i_am_left) return;                       // the left leaf's thread handles the pair
+        } else {
+            __threadfence();                              // my record is visible before I announce myself
+            if (atomicAdd(&visit[node], 1u) == 0u) return;    // first arrival: the sibling's thread will carry on
+            asm volatile("" ::: "memory");                // keep the sibling loads below the atomic in program order
+        }
         double slo[3], shi[3], shm;
         if (sib_leaf) {
             slo[0] = shi[0] = x[sib]; slo[1] = shi[1] = y[sib]; slo[2] = shi[2] = z[sib];
