@@ -140,8 +140,14 @@ static int cache_build(sph_ctx* c) {
             return fail(c, SPH_ERR_CAP, "%u leaf groups have more than 65535 candidates (16-bit local index)",
                         s.n_cand_overflow);
         if (getenv("SPH_DEBUG"))
-            fprintf(stderr, "[sph] groups %u nc_max %u fallback %u nbr_min %u nbr_max %u lists %llu candidates %llu\n",
-                    s.n_groups, s.nc_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.cslot_cursor);
+            fprintf(stderr, "[sph] groups %u nc_max %u fallback %u nbr_min %u nbr_max %u lists %llu candidates %llu chunk %u shared %u overflow %u\n",
+                    s.n_groups, s.nc_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.cslot_cursor, c->last_chunk,
+                    s.n_chunks_shared, s.n_chunks_overflow);
+        if (c->last_chunk > 1) {
+            const uint64_t chunks = ((uint64_t)s.n_groups + c->last_chunk - 1) / c->last_chunk;
+            if ((uint64_t)s.n_chunks_shared * 10 < chunks * 8 || (uint64_t)s.n_chunks_overflow * 50 > chunks)
+                c->share_disabled = true;
+        }
         c->n_groups = s.n_groups;
         c->nc_max = s.nc_max;
         c->n_neigh = s.n_neigh;

@@ -63,6 +63,8 @@ struct DevScalars {
     unsigned long long cslot_cursor; // candidate-pool entries handed out (each group's array padded to 4)
     unsigned int nc_max;             // largest candidate count of any group
     unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
+    unsigned int n_chunks_shared;    // traversal chunks that shared one walk / whose shared walk overflowed
+    unsigned int n_chunks_overflow;
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
 };
@@ -129,6 +131,8 @@ struct sph_ctx {
     double t = 0.0;
     int64_t launches = 0;
     bool have_cfl_dt = false;
+    bool share_disabled = false;        // traversal: shared walks switched off (too few chunks could share)
+    uint32_t last_chunk = 1;
     bool uniform_mass = false;          // all particle masses equal (density kernel variant)
 
     std::vector<sph::TimerRec> timers;

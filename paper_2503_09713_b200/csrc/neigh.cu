@@ -2,7 +2,10 @@
 // (Alg. 4; Alg. 5; two-stage idea PAPER.md:1164-1166; criteria of App. E,
 // PAPER.md:1217-1229, with the cache tolerance chi, reading A2).
 //
-// One warp per leaf group (<= 32 Morton-contiguous particles; lane = query particle), ONE pass:
+// One warp per leaf group (<= 32 Morton-contiguous particles; lane = query particle), ONE pass. A warp takes kShare
+// consecutive groups at a time and walks the tree once for their common box, collecting the bucket nodes within
+// reach; each group then only re-tests those buckets against its own box (stage 1 is mostly the thinly populated
+// top of the tree, and consecutive groups share it).
 //   Stage 1: the warp pops up to 32 nodes at a time from a shared-memory stack; each lane tests one node's box,
 //     enlarged by R_kern chi max(hmax_group, hmax_node), against the group's box under the periodic minimum image
 //     (group-group criterion). Passing nodes with <= 32 particles become candidate buckets (slot
@@ -21,6 +24,8 @@
 //     allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed). A group whose
 //     buffers overflow (a list longer than kHitCap, more than kScrCap candidates) allocates from its exact
 //     counts and walks a second time writing directly.
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace sph {
@@ -32,6 +37,8 @@ constexpr int kPendCap = 64;             // candidate buckets buffered before st
 constexpr int kHitCap = 112;             // buffered hits per lane
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
 constexpr int kHitStride = kHitCap + kHitSlack + 2;   // in u16: 73 words per lane row (odd: rows start in distinct banks)
+constexpr int kShare = 4;               // consecutive groups that share one tree walk
+constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
 constexpr int kScrCap = 2048;            // candidate slots buffered per group (global scratch row of the warp)
 constexpr uint32_t kLeafBit = 0x80000000u;
 constexpr uint32_t kWrapBit = 0x80000000u;
@@ -47,6 +54,7 @@ struct TravWarpSmem {
     uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
     double2 cxy[32], czr[32];                 // staged candidates (compacted): {x, y}, {z, (R_kern chi h)^2}
     uint32_t cid[32];                         // their indices in the group's candidate array
+    uint32_t ub[kUbCap];                      // bucket nodes within reach of the kShare groups' common box
     uint16_t hits[32 * kHitStride];
 };
 
@@ -203,7 +211,113 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
     }
 }
 
-// one complete walk of the tree for the group described by G
+// One node against the box / hmax of G: group-group criterion on the squared box-box gap under the
+// minimum image, conservative under rounding (tiny pad); `wrap` says whether any (query, candidate) separation can
+// exceed L/2 on a periodic axis (exact: rounding is monotone). Entry e = internal node index, or leaf slot | kLeafBit.
+struct NodeHit { bool pass, small, wrap; uint32_t rlo, rhi, split; };
+__device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, const double* __restrict__ x,
+                                             const double* __restrict__ y, const double* __restrict__ z,
+                                             const double* __restrict__ h, const NodeRec* __restrict__ nodes,
+                                             const TravBox& tb, double rk_chi) {
+    NodeHit r;
+    double blo[3], bhi[3], bhm;
+    r.split = 0u;
+    if (e & kLeafBit) {
+        r.rlo = r.rhi = e & ~kLeafBit;
+        blo[0] = bhi[0] = x[r.rlo]; blo[1] = bhi[1] = y[r.rlo]; blo[2] = bhi[2] = z[r.rlo];
+        bhm = h[r.rlo];
+        r.small = true;
+    } else {
+        const double2* p = reinterpret_cast<const double2*>(nodes + e);
+        const double2 v0 = __ldg(p), v1 = __ldg(p + 1), v2 = __ldg(p + 2), v3 = __ldg(p + 3);
+        blo[0] = v0.x; blo[1] = v0.y; blo[2] = v1.x; bhi[0] = v1.y; bhi[1] = v2.x; bhi[2] = v2.y;
+        bhm = v3.x;
+        const long long ints = __double_as_longlong(v3.y);
+        const int32_t other = (int32_t)(ints & 0xffffffffll);
+        r.split = (uint32_t)(ints >> 32);
+        r.rlo = min(e, (uint32_t)other);
+        r.rhi = max(e, (uint32_t)other);
+        r.small = (r.rhi - r.rlo + 1) <= (uint32_t)kGroup;
+    }
+    const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
+    const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
+    const double ggy = axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]);
+    const double ggz = axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]);
+    r.pass = ggx * ggx + ggy * ggy + ggz * ggz <= ext * ext;
+    r.wrap = (tb.periodic[0] && (dmax(G.gxh, bhi[0]) - dmin(G.gxl, blo[0]) > tb.halfL[0])) ||
+             (tb.periodic[1] && (dmax(G.gyh, bhi[1]) - dmin(G.gyl, blo[1]) > tb.halfL[1])) ||
+             (tb.periodic[2] && (dmax(G.gzh, bhi[2]) - dmin(G.gzl, blo[2]) > tb.halfL[2]));
+    return r;
+}
+
+// Walk of the tree for a box U that encloses several consecutive groups: collects the bucket nodes (<= 32
+// particles) within reach of U into s.ub. Every bucket a member group needs is among them: the group's box lies
+// inside U and its hmax is not larger, every operation of the test is monotone, so a node that passes the group's
+// test passes U's, and so do all its ancestors. Returns the number of buckets, or -1 if s.ub overflowed.
+__device__ __forceinline__ int walk_collect(TravWarpSmem& s, const GroupCtx& U, unsigned lane, unsigned lt, int64_t N,
+                                            const double* __restrict__ x, const double* __restrict__ y,
+                                            const double* __restrict__ z, const double* __restrict__ h,
+                                            const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
+    int sp = 1, nu = 0;
+    __syncwarp();
+    if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
+    __syncwarp();
+    while (sp > 0) {
+        int npop = min(sp, 32);
+        if (sp > kStackCap - kStackSlack) npop = 1;
+        const bool have = (int)lane < npop;
+        const uint32_t e = have ? s.stack[sp - 1 - lane] : 0u;
+        sp -= npop;
+        __syncwarp();
+        NodeHit r;
+        r.pass = false; r.small = false;
+        if (have) r = node_test(e, U, x, y, z, h, nodes, tb, rk_chi);
+        const bool push = r.pass && !r.small, emit = r.pass && r.small;
+        const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
+        if (push) {
+            const int at = sp + 2 * __popc(pm & lt);
+            s.stack[at] = (r.rhi == r.split + 1) ? (kLeafBit | (r.split + 1)) : (r.split + 1);
+            s.stack[at + 1] = (r.rlo == r.split) ? (kLeafBit | r.split) : r.split;
+        }
+        sp += 2 * __popc(pm);
+        if (nu + __popc(em) > kUbCap) return -1;
+        if (emit) s.ub[nu + __popc(em & lt)] = e;
+        nu += __popc(em);
+        __syncwarp();
+    }
+    return nu;
+}
+
+// One group's buckets out of the collected ones (the same test with the group's own box), then stage 2.
+template <bool DIRECT>
+__device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, unsigned lane, unsigned lt,
+                                       const double* __restrict__ x, const double* __restrict__ y,
+                                       const double* __restrict__ z, const double* __restrict__ h,
+                                       const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
+    G.nhit = 0u; G.wpos = 0u; G.ncs = 0u; G.anywrap = false;
+    int nb = 0;
+    __syncwarp();
+    for (int base = 0; base < nu; base += 32) {
+        const bool have = base + (int)lane < nu;
+        NodeHit r;
+        r.pass = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u;
+        if (have) r = node_test(s.ub[base + lane], G, x, y, z, h, nodes, tb, rk_chi);
+        const unsigned em = __ballot_sync(0xffffffffu, r.pass);
+        if (r.pass) {
+            const int at = nb + __popc(em & lt);
+            s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
+            s.pn[at] = r.rhi - r.rlo + 1;
+        }
+        nb += __popc(em);
+        __syncwarp();
+        if (nb > kPendCap - 32) { stage2<DIRECT>(s, G, nb, lane, lt, x, y, z, h, tb, rk_chi); nb = 0; }
+    }
+    __syncwarp();
+    stage2<DIRECT>(s, G, nb, lane, lt, x, y, z, h, tb, rk_chi);
+    __syncwarp();
+}
+
+// one complete walk of the tree for the group described by G (used when the shared walk overflowed s.ub)
 template <bool DIRECT>
 __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane, unsigned lt, int64_t N,
                                      const double* __restrict__ x, const double* __restrict__ y,
@@ -221,50 +335,21 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
         const uint32_t e = have ? s.stack[sp - 1 - lane] : 0u;
         sp -= npop;
         __syncwarp();
-        bool pass = false, small = false, wrap = false;
-        uint32_t rlo = 0, rhi = 0, split = 0;
-        if (have) {
-            double blo[3], bhi[3], bhm;
-            if (e & kLeafBit) {
-                rlo = rhi = e & ~kLeafBit;
-                blo[0] = bhi[0] = x[rlo]; blo[1] = bhi[1] = y[rlo]; blo[2] = bhi[2] = z[rlo];
-                bhm = h[rlo];
-                small = true;
-            } else {
-                const double2* p = reinterpret_cast<const double2*>(nodes + e);
-                const double2 v0 = __ldg(p), v1 = __ldg(p + 1), v2 = __ldg(p + 2), v3 = __ldg(p + 3);
-                blo[0] = v0.x; blo[1] = v0.y; blo[2] = v1.x; bhi[0] = v1.y; bhi[1] = v2.x; bhi[2] = v2.y;
-                bhm = v3.x;
-                const long long ints = __double_as_longlong(v3.y);
-                const int32_t other = (int32_t)(ints & 0xffffffffll);
-                split = (uint32_t)(ints >> 32);
-                rlo = min(e, (uint32_t)other);
-                rhi = max(e, (uint32_t)other);
-                small = (rhi - rlo + 1) <= (uint32_t)kGroup;
-            }
-            // group-group criterion, conservative under rounding (tiny pad)
-            const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
-            const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
-            const double ggy = axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]);
-            const double ggz = axis_gap(G.gzl, G.gzh, blo[2], bhi[2], tb.L[2], tb.periodic[2]);
-            pass = ggx * ggx + ggy * ggy + ggz * ggz <= ext * ext;
-            // can any (query, candidate) separation exceed L/2 on a periodic axis? (exact: rounding is monotone)
-            wrap = (tb.periodic[0] && (dmax(G.gxh, bhi[0]) - dmin(G.gxl, blo[0]) > tb.halfL[0])) ||
-                   (tb.periodic[1] && (dmax(G.gyh, bhi[1]) - dmin(G.gyl, blo[1]) > tb.halfL[1])) ||
-                   (tb.periodic[2] && (dmax(G.gzh, bhi[2]) - dmin(G.gzl, blo[2]) > tb.halfL[2]));
-        }
-        const bool push = pass && !small, emit = pass && small;
+        NodeHit r;
+        r.pass = false; r.small = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u; r.split = 0u;
+        if (have) r = node_test(e, G, x, y, z, h, nodes, tb, rk_chi);
+        const bool push = r.pass && !r.small, emit = r.pass && r.small;
         const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
         if (push) {
             const int at = sp + 2 * __popc(pm & lt);
-            s.stack[at] = (rhi == split + 1) ? (kLeafBit | (split + 1)) : (split + 1);
-            s.stack[at + 1] = (rlo == split) ? (kLeafBit | split) : split;
+            s.stack[at] = (r.rhi == r.split + 1) ? (kLeafBit | (r.split + 1)) : (r.split + 1);
+            s.stack[at + 1] = (r.rlo == r.split) ? (kLeafBit | r.split) : r.split;
         }
         sp += 2 * __popc(pm);
         if (emit) {
             const int at = nb + __popc(em & lt);
-            s.plo[at] = rlo | (wrap ? kWrapBit : 0u);
-            s.pn[at] = rhi - rlo + 1;
+            s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
+            s.pn[at] = r.rhi - r.rlo + 1;
         }
         nb += __popc(em);
         __syncwarp();
@@ -287,10 +372,10 @@ __device__ __forceinline__ uint32_t warp_max_u32(uint32_t v) {
     return v;
 }
 
-__global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
+__global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
     int64_t N, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ h, const NodeRec* __restrict__ nodes, const uint32_t* __restrict__ grp_lo,
-    TravBox tb, double rk_chi, TravOut out, uint32_t* work_counter, DevScalars* sc) {
+    TravBox tb, double rk_chi, TravOut out, uint32_t* work_counter, DevScalars* sc, uint32_t chunk) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TravWarpSmem& s = reinterpret_cast<TravWarpSmem*>(smem_raw)[threadIdx.x >> 5];
     const unsigned lane = lane_id();
@@ -300,10 +385,39 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
     uint32_t* const scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
 
     for (;;) {
-        uint32_t g = 0;
-        if (lane == 0) g = atomicAdd(work_counter, 1u);     // dynamic work distribution (skewed list lengths)
-        g = __shfl_sync(0xffffffffu, g, 0);
-        if (g >= n_groups) break;
+        uint32_t g0 = 0;
+        if (lane == 0) g0 = atomicAdd(work_counter, chunk);   // dynamic work distribution, chunk = 1 or kShare groups
+        g0 = __shfl_sync(0xffffffffu, g0, 0);
+        if (g0 >= n_groups) break;
+        const uint32_t ng = min(chunk, n_groups - g0);
+        // ---- one walk for the common box of the kShare consecutive groups (a contiguous slot range) ----
+        // Sharing pays only if the groups are neighbours in space as well as in Morton order: compare the volume
+        // within reach of the common box with the largest one of a member group.
+        int nu = -1;
+        if (ng > 1u) {
+            GroupCtx U;
+            U.gxl = U.gyl = U.gzl = 1e300; U.gxh = U.gyh = U.gzh = -1e300; U.ghm = 0.0;
+            double vmax = 0.0, vmin = 1e300;
+            for (uint32_t g = g0; g < g0 + ng; ++g) {
+                const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
+                const uint32_t a = glo + (lane < nq ? lane : 0u);
+                const double xi = x[a], yi = y[a], zi = z[a], hi = h[a];
+                const double xl = warp_min(xi), xh = warp_max(xi), yl = warp_min(yi), yh = warp_max(yi);
+                const double zl = warp_min(zi), zh = warp_max(zi), hm = warp_max(hi);
+                const double rr = 2.0 * rk_chi * hm;
+                const double vg = (xh - xl + rr) * (yh - yl + rr) * (zh - zl + rr);
+                vmax = dmax(vmax, vg); vmin = dmin(vmin, vg);
+                U.gxl = dmin(U.gxl, xl); U.gxh = dmax(U.gxh, xh); U.gyl = dmin(U.gyl, yl); U.gyh = dmax(U.gyh, yh);
+                U.gzl = dmin(U.gzl, zl); U.gzh = dmax(U.gzh, zh); U.ghm = dmax(U.ghm, hm);
+            }
+            const double rr = 2.0 * rk_chi * U.ghm;
+            const double vu = (U.gxh - U.gxl + rr) * (U.gyh - U.gyl + rr) * (U.gzh - U.gzl + rr);
+            if (vu <= 3.0 * vmax && vmax <= 4.0 * vmin) {
+                nu = walk_collect(s, U, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
+                if (lane == 0) atomicAdd(nu >= 0 ? &sc->n_chunks_shared : &sc->n_chunks_overflow, 1u);
+            }
+        }
+        for (uint32_t g = g0; g < g0 + ng; ++g) {
         const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
         GroupCtx G;
         const bool qv = lane < nq;
@@ -324,7 +438,8 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
         if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
 
-        walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
+        if (nu >= 0) refine<false>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
+        else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
         // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and candidate slots ----
         const uint32_t nhit = qv ? G.nhit : 0u;
@@ -374,13 +489,15 @@ __global__ void __launch_bounds__(kTravWarps * 32) k_traverse(
                 G.lptr = out.lists + my_start;
                 G.cptr = out.cslot + bbase;
                 G.can_write = true;
-                walk<true>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
+                if (nu >= 0) refine<true>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
+                else walk<true>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
                 if (lane == 0) atomicAdd(&sc->n_fallback, 1u);
             }
         }
         if (nc > 65535u && lane == 0) atomicAdd(&sc->n_cand_overflow, 1u);
         if (qv) { mn = min(mn, nhit); mx = max(mx, nhit); }
         ncmax = max(ncmax, nc);
+        }   // groups of the chunk
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -397,7 +514,7 @@ __global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc) {
     *work_counter = 0u;
     sc->nbr_min = 0xffffffffu; sc->nbr_max = 0u;
     sc->list_cursor = 0ull; sc->cslot_cursor = 0ull; sc->n_neigh = 0ull;
-    sc->nc_max = 0u; sc->n_cand_overflow = 0u; sc->n_fallback = 0u;
+    sc->nc_max = 0u; sc->n_cand_overflow = 0u; sc->n_chunks_shared = 0u; sc->n_chunks_overflow = 0u; sc->n_fallback = 0u;
 }
 
 constexpr int kTravBlocks = 148 * 2;     // persistent grid: two CTAs per SM (shared-memory bound)
@@ -429,8 +546,12 @@ int launch_traverse(sph_ctx* c) {
     const int64_t warps_needed = (c->N + 31) / 32;
     unsigned blocks = (unsigned)min((int64_t)kTravBlocks, (warps_needed + kTravWarps - 1) / kTravWarps);
     if (blocks == 0) blocks = 1;
+    // Shared walks (kShare consecutive groups per warp) pay when there are many groups per warp and the groups of a
+    // chunk are alike; api.cu switches them off for good if the last pass shared too few chunks.
+    const uint32_t chunk = (!c->share_disabled && c->n_groups >= (int64_t)32 * kTravBlocks * kTravWarps) ? kShare : 1u;
+    c->last_chunk = chunk;
     k_traverse<<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
-                                                             c->grp_lo, tb, rk_chi, out, wc, c->d_sc);
+                                                             c->grp_lo, tb, rk_chi, out, wc, c->d_sc, chunk);
     c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
