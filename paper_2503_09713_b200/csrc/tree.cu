@@ -16,7 +16,7 @@ __device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int64
 
 // one thread per internal node i in [0, N-2]
 __global__ void __launch_bounds__(256) k_karras(int64_t N, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
-                                                int32_t* __restrict__ parent) {
+                                                int32_t* __restrict__ parent, uint32_t* __restrict__ gflag) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N - 1) return;
     const uint64_t ki = key[i];
@@ -42,21 +42,13 @@ __global__ void __launch_bounds__(256) k_karras(int64_t N, const uint64_t* __res
     parent[(lo == gamma) ? (N - 1 + gamma) : gamma] = (int32_t)i;
     parent[(hi == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1)] = (int32_t)i;
     if (i == 0) parent[0] = -1;
-}
-
-// leaf groups: children of nodes with more than kGroup particles that themselves hold <= kGroup
-__global__ void __launch_bounds__(256) k_group_flags(int64_t N, const NodeRec* __restrict__ nodes, uint32_t* __restrict__ gflag) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N - 1) return;
-    int32_t other = nodes[i].other, split = nodes[i].split;
-    int64_t lo = min((int64_t)other, i), hi = max((int64_t)other, i);
+    // leaf groups: children of nodes with more than kGroup particles that themselves hold <= kGroup
     if (hi - lo + 1 <= kGroup) {
         if (i == 0) gflag[0] = 1u;   // the whole tree is one group
-        return;
+    } else {
+        if (gamma - lo + 1 <= kGroup) gflag[lo] = 1u;        // left child covers [lo, gamma]
+        if (hi - gamma <= kGroup) gflag[gamma + 1] = 1u;     // right child covers [gamma + 1, hi]
     }
-    // left child covers [lo, split], right child [split+1, hi]
-    if (split - lo + 1 <= kGroup) gflag[lo] = 1u;
-    if (hi - split <= kGroup) gflag[split + 1] = 1u;
 }
 
 __global__ void __launch_bounds__(256) k_group_fill(int64_t N, const uint32_t* __restrict__ gflag,
@@ -129,9 +121,8 @@ int launch_tree(sph_ctx* c) {
     const int64_t N = c->N;
     SPH_CUDA(c, cudaMemsetAsync(c->gflag, 0, (size_t)N * sizeof(uint32_t), c->stream));
     if (N >= 2) {
-        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent);
-        k_group_flags<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->nodes, c->gflag);
-        c->launches += 2;
+        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag);
+        c->launches++;
     } else {
         k_single_group<<<1, 1, 0, c->stream>>>(c->gflag);
         c->launches++;
