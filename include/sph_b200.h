@@ -100,6 +100,11 @@ typedef struct {
   double dt;             /* current CFL timestep (G8)                                        */
   double t;              /* simulated time                                                   */
   int64_t bytes_allocated;
+  /* neighbour-cache diagnostics of the last traversal pass */
+  int32_t cand_max;        /* largest candidate array of any leaf group                                  */
+  int32_t groups_fallback; /* groups that overflowed their buffers and were walked a second time          */
+  int32_t chunks_shared;   /* chunks of consecutive groups that shared one tree walk (0: sharing off)     */
+  int32_t share_chunk;     /* groups per chunk used by the last pass (1 or 4)                             */
 } sph_stats;
 
 void sph_default_params(sph_params* p);

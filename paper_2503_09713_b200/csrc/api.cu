@@ -538,6 +538,8 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->nbr_mean = c->N ? (double)c->n_neigh / (double)c->N : 0.0;
     out->h_iter_max = (int32_t)s.h_iter_max; out->restarts = c->restarts_last; out->steps = c->steps;
     out->kernel_launches = c->launches; out->dt = s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
+    out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
+    out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
     return SPH_OK;
 }
 

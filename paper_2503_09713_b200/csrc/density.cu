@@ -2,8 +2,8 @@
 // PAPER.md:1235-1239; lambda clamp and chi tolerance PAPER.md:1245; sign safeguard DESIGN.md reading A5b), then
 // rho = m (hfact/h)^3 and Omega (Eq. 7) at the converged h.
 //
-// One CTA of eight warps per leaf group. The group's candidate array (the slot ranges of its bucket table) is
-// staged once into shared memory with coalesced loads: x, y, z, m of every candidate. Every particle of the group
+// One CTA of eight warps per leaf group. The group's candidate array is staged once into shared memory with
+// cp.async copies: x, y, z, m of every candidate (groups with more candidates than fit gather from global memory). Every particle of the group
 // is owned by one octet (8 lanes): warp w, octet o -> particle 4 w + o, so a warp iterates four independent Newton
 // solves at once and the scalar update is executed 8-fold instead of 32-fold redundantly. The octet's lanes split
 // the particle's neighbour list (16-bit indices into the staged candidates); r_ab and m_b are computed once and
@@ -52,21 +52,25 @@ struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 
 // UNIM: every candidate of the group has the same mass (checked while staging): the mass factors out of the sums
 // and the per-neighbour mass registers disappear.
-template <bool WRAP, bool UNIM>
+// GLOB: the candidate array is too large to stage; sx, sy, sz, sm are the global field arrays and a candidate index
+// is translated through the group's candidate array cs first.
+template <bool WRAP, bool UNIM, bool GLOB>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
+                                            const uint32_t* __restrict__ cs,
                                             const uint16_t* __restrict__ li, const uint32_t (&idx)[kRegChunks / 2],
                                             int n, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
     double r[kRegChunks], mb[UNIM ? 1 : kRegChunks];
-    const double m0 = sm[0];
+    const double m0 = ma;                              // UNIM: every particle has this mass
 #pragma unroll
     for (int c = 0; c < kRegChunks; ++c) {
         const int k = c * 8 + (int)sl;
         r[c] = 1e100;                                  // q >> 2 (finite): outside the kernel support, contributes 0
         if (!UNIM) mb[c] = 0.0;
         if (k < n) {
-            const uint32_t b = (idx[c >> 1] >> (16 * (c & 1))) & 0xffffu;
+            uint32_t b = (idx[c >> 1] >> (16 * (c & 1))) & 0xffffu;
+            if (GLOB) b = cs[b];
             r[c] = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db);
             if (!UNIM) mb[c] = sm[b];
         }
@@ -88,7 +92,8 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
             }
         }
         for (int k = kRegChunks * 8 + (int)sl; k < n; k += 8) {      // long lists: re-gather from smem
-            const uint32_t b = li[k];
+            uint32_t b = li[k];
+            if (GLOB) b = cs[b];
             double qq = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, df;
             const double mm = UNIM ? 1.0 : sm[b];
             m4(qq, f, df);
@@ -139,7 +144,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     out.it = it;
 }
 
-template <bool UNIM>
+template <bool UNIM, bool GLOB>
 __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
@@ -171,9 +176,13 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     const int n = pv ? (int)cnt[a] : 0;
 
     // ---- stage the candidate array (slots are mostly runs of consecutive indices: coalesced sectors) ----
-    for (uint32_t c = threadIdx.x; c < nc; c += kDensWarps * 32) {
-        const uint32_t s = cs[c];
-        cp_async8(sx + c, x + s); cp_async8(sy + c, y + s); cp_async8(sz + c, z + s); cp_async8(sm + c, m + s);
+    if (!GLOB) {
+        for (uint32_t c = threadIdx.x; c < nc; c += kDensWarps * 32) {
+            const uint32_t s = cs[c];
+            cp_async8(sx + c, x + s); cp_async8(sy + c, y + s); cp_async8(sz + c, z + s); cp_async8(sm + c, m + s);
+        }
+    } else {
+        sx = const_cast<double*>(x); sy = const_cast<double*>(y); sz = const_cast<double*>(z); sm = const_cast<double*>(m);
     }
     // the first 96 list entries of the octet's particle (two 16-bit indices per register), in flight together with
     // the staging copies
@@ -188,8 +197,8 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     __syncthreads();
 
     DensOut o;
-    if (gwrap) octet_solve<true, UNIM>(xa, ya, za, ma, h0, pv, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
-    else octet_solve<false, UNIM>(xa, ya, za, ma, h0, pv, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    if (gwrap) octet_solve<true, UNIM, GLOB>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    else octet_solve<false, UNIM, GLOB>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
 
     if (pv && sl == 0u) {
         hout[a] = o.h;
@@ -210,11 +219,20 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
 
 __global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; }
 
+template <bool UNIM, bool GLOB>
+static void density_launch(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
+                           uint32_t hi) {
+    k_density<UNIM, GLOB><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+        c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db, dp,
+        ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
+    c->launches++;
+}
+
 int launch_density(sph_ctx* c) {
     static bool attr_set = false;
     if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        SPH_CUDA(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        SPH_CUDA(c, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        SPH_CUDA(c, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_set = true;
     }
     DensBox db;
@@ -225,31 +243,26 @@ int launch_density(sph_ctx* c) {
     }
     DensPar dp;
     dp.hfact = c->p.hfact; dp.chi = c->p.chi; dp.lambda = c->p.lambda; dp.eps_h = c->p.eps_h; dp.max_iter = c->p.max_h_iter;
-    if ((size_t)c->nc_max * 4 * sizeof(double) > 227 * 1024)
-        return fail(c, SPH_ERR_CAP, "a leaf group has %u candidates: more than the density kernel can stage (%d)",
-                    c->nc_max, 227 * 1024 / 32);
     k_density_reset<<<1, 1, 0, c->stream>>>(c->d_sc);
     c->launches++;
-    // The staged candidate array sizes the CTA's shared memory, hence the occupancy: groups are served in two size
-    // classes (a CTA whose group belongs to the other class exits at once), so that a few crowded groups (density
-    // jumps, disc mid-plane) do not cost everyone else their occupancy. One launch when all groups are small.
-    const uint32_t kSmall = 768;
-    for (int cls = 0; cls < 2; ++cls) {
-        const uint32_t lo = cls == 0 ? 0u : kSmall, hi = cls == 0 ? kSmall : 0x7fffffffu;
-        if (cls == 1 && c->nc_max <= kSmall) break;
-        // nc = 0 cannot occur (a particle is its own neighbour); lo = 0 therefore excludes nothing in class 0
-        const uint32_t ncap = ((cls == 0 ? (c->nc_max < kSmall ? c->nc_max : kSmall) : c->nc_max) + 31u) & ~31u;
+    // The staged candidate array sizes the CTA's shared memory, hence the occupancy: groups are served in size
+    // classes (a CTA whose group belongs to another class exits at once), so that a few crowded groups (density
+    // jumps, disc mid-plane) do not cost everyone else their occupancy: up to kSmall candidates; up to kStage (what
+    // fits in shared memory at all); beyond that, a variant that gathers from global memory (poor initial h only).
+    const uint32_t kSmall = 768, kStage = 227 * 1024 / 32;
+    const uint32_t bounds[4] = {0u, kSmall, kStage, 0x7fffffffu};
+    for (int cls = 0; cls < 3; ++cls) {
+        const uint32_t lo = bounds[cls], hi = bounds[cls + 1];
+        if (c->nc_max <= lo) break;                      // nc = 0 cannot occur (a particle is its own neighbour)
+        const uint32_t ncap = cls == 2 ? 0u : ((c->nc_max < hi ? c->nc_max : hi) + 31u) & ~31u;
         const size_t smem = (size_t)ncap * 4 * sizeof(double);
-        // all masses equal (checked once at init): the kernel variant without per-neighbour mass registers
-        if (c->uniform_mass)
-            k_density<true><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-                c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists,
-                db, dp, ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
-        else
-            k_density<false><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-                c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists,
-                db, dp, ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
-        c->launches++;
+        if (c->uniform_mass) {      // all masses equal (checked once at init): no per-neighbour mass registers
+            if (cls == 2) density_launch<true, true>(c, smem, db, dp, ncap, lo, hi);
+            else density_launch<true, false>(c, smem, db, dp, ncap, lo, hi);
+        } else {
+            if (cls == 2) density_launch<false, true>(c, smem, db, dp, ncap, lo, hi);
+            else density_launch<false, false>(c, smem, db, dp, ncap, lo, hi);
+        }
     }
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -548,7 +548,9 @@ int launch_traverse(sph_ctx* c) {
     if (blocks == 0) blocks = 1;
     // Shared walks (kShare consecutive groups per warp) pay when there are many groups per warp and the groups of a
     // chunk are alike; api.cu switches them off for good if the last pass shared too few chunks.
-    const uint32_t chunk = (!c->share_disabled && c->n_groups >= (int64_t)32 * kTravBlocks * kTravWarps) ? kShare : 1u;
+    // SPH_FORCE_SHARE=1 (tests) forces shared walks whatever the problem size.
+    const bool force = getenv("SPH_FORCE_SHARE") != nullptr;
+    const uint32_t chunk = (force || (!c->share_disabled && c->n_groups >= (int64_t)32 * kTravBlocks * kTravWarps)) ? kShare : 1u;
     c->last_chunk = chunk;
     k_traverse<<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
                                                              c->grp_lo, tb, rk_chi, out, wc, c->d_sc, chunk);

@@ -368,3 +368,38 @@ def test_c1_sod_full_size_sampled_parity():
     _sampled_parity(w, sim, (0.0, 0.0, 0.0), 0.03)
     _sampled_parity(w, sim, (0.5, 0.125, -0.125), 0.03)          # the periodic seam, a box corner
     sim.close()
+
+
+@pytest.mark.parametrize("make", [
+    lambda: W.cube(24, jitter=0.1, vel_amp=0.01, seed=5),
+    lambda: W.random_cloud(6000, seed=13),
+    lambda: W.sod(16, 12),
+], ids=["cube24", "cloud", "sod_small"])
+def test_shared_walk_is_exact(make, monkeypatch):
+    """Shared tree walks (four consecutive groups walk once for their common box, DESIGN.md 6 a4) are normally
+    used only for large problems; forced here so that the complete stage parity, bit-exact neighbour sets included,
+    covers that path too."""
+    monkeypatch.setenv("SPH_FORCE_SHARE", "1")
+    w = make()
+    sim = _sim(w)
+    st = sim.stats()
+    assert st["share_chunk"] == 4
+    _stage_parity(w, sim)
+    sim.step_leapfrog()
+    sim.close()
+
+
+def test_density_size_classes_and_fallback_paths():
+    """A clustered cloud has groups with few and with many candidates (both density size classes run) and lists
+    longer than the traversal's hit buffer (groups walked a second time writing directly)."""
+    w = W.random_cloud(20000, seed=21)
+    w.h0 = w.h0 * 1.6
+    from paper_2503_09713_b200 import binding as B
+    sim = B.Sim.from_workload(w, white_step=False)
+    sim.build_tree()
+    st = sim.stats()
+    assert st["cand_max"] > 768 and st["groups_fallback"] > 0 and st["nbr_max"] > 112
+    sim.close()
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    sim.close()
