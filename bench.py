@@ -59,6 +59,8 @@ def make_workload(name: str, seed_offset: int = 0):
         return W.cube(n, jitter=0.1, seed=seed, steps=5, name=f"C2-recipe uniform periodic cube {n}^3")
     if name == "sod":
         return W.config(1)
+    if name.startswith("sedov"):   # the paper's timing set-up: both CFL numbers 1e-3
+        return W.sedov(int(name[5:] or 256), cfl=1e-3, name=f"Sedov-Taylor blast, HCP lattice, n_side {name[5:] or 256}")
     if name.startswith("disc"):
         n = int(name[4:] or 10_000_000)
         return W.disc(n, seed=seed)

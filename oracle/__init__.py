@@ -63,6 +63,9 @@ def make_params(gamma=5.0 / 3.0, hfact=1.2, chi=1.1, lam=1.2, eps_h=1e-6, alpha_
 
 def workload_box_params(w, **kw):
     """Box and Params for a ``workloads.Workload`` (duck-typed: the oracle does not import that module)."""
+    cfl = getattr(w, "cfl", None)
+    if cfl is not None:
+        kw = dict(dict(c_cour=cfl[0], c_force=cfl[1]), **kw)
     return (make_box(w.box_lo, w.box_hi, w.periodic),
             make_params(gamma=w.gamma, hfact=w.hfact, eos_isothermal=w.eos_isothermal, point_mass=w.point_mass, **kw))
 

@@ -119,6 +119,8 @@ def params_for(w, **kw) -> Params:
         extra.update(eos=1, cs0=w.eos_isothermal[0], r0=w.eos_isothermal[1], q=w.eos_isothermal[2])
     if w.point_mass is not None:
         extra.update(GM=w.point_mass[0], soft=w.point_mass[1], centre=w.point_mass[2])
+    if getattr(w, "cfl", None) is not None:
+        extra.update(c_cour=w.cfl[0], c_force=w.cfl[1])
     extra.update(kw)
     return default_params(**extra)
 

@@ -51,6 +51,7 @@ class Workload:
     eos_isothermal: tuple | None = None  # (cs0, r0, q): cs = cs0 * (R / r0) ** -q
     point_mass: tuple | None = None  # (GM, softening, (cx, cy, cz))
     steps: int = 1
+    cfl: tuple | None = None  # (C_cour, C_force) if not the defaults (Sedov blast)
 
     @property
     def n(self) -> int:
@@ -145,6 +146,39 @@ def disc(n: int = 10_000_000, seed: int = DEFAULT_SEED, hfact: float = 1.2, step
     return Workload(name or f"disc{n}", np.ascontiguousarray(pos), np.ascontiguousarray(vel), mass, u, h0,
                     (-12.0, -12.0, -12.0), (12.0, 12.0, 12.0), (0, 0, 0), 1.0, hfact,
                     eos_isothermal=(cs0, 2.0, 0.25), point_mass=(GM, eps, (0.0, 0.0, 0.0)), steps=steps)
+
+
+def sedov(n_side: int = 128, E0: float = 1.0, cfl: float = 0.1, gamma: float = 5.0 / 3.0, hfact: float = 1.2,
+          steps: int = 5, name: str | None = None) -> Workload:
+    """Sedov-Taylor blast set-up, the paper's own performance benchmark (SURVEY.md 8(f)
+    item 2): periodic box [-0.6, 0.6]^3, rho = 1, v = 0, particles on a close-packed (HCP) lattice with ``n_side``
+    sites along x (row and layer counts rounded to even numbers and the y, z spacings stretched by a few per cent,
+    less as n_side grows, so that the lattice is periodic), equal masses, and the energy E0 = 1 injected at the centre as u_a = E0 W(r_a, 2 h0)
+    with the M4 kernel and h0 = hfact (m/rho)^(1/3) (the relaxed h of the lattice to 3e-4); u = 0 elsewhere.
+    ``cfl`` sets both C_cour and C_force (0.1 for the physics run, 1e-3 for the paper's timing run). The leapfrog
+    corrector re-cycle (G6-G10) is not built, so this is for short timing / parity runs."""
+    L = 1.2
+    nx = int(n_side)
+    dx = L / nx
+    ny = 2 * max(1, round(L / (dx * math.sqrt(3.0) / 2.0) / 2.0))
+    nz = 2 * max(1, round(L / (dx * math.sqrt(6.0) / 3.0) / 2.0))
+    dy, dz = L / ny, L / nz
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    x = (i + 0.5 * (j % 2) + 0.5 * (k % 2) + 0.25) * dx
+    y = (j + (k % 2) / 3.0 + 0.25) * dy
+    z = (k + 0.25) * dz
+    pos = np.stack([np.mod(x.ravel(), L), np.mod(y.ravel(), L), np.mod(z.ravel(), L)]) - 0.5 * L
+    pos = np.ascontiguousarray(np.clip(pos, -0.5 * L, np.nextafter(0.5 * L, 0.0)))
+    n = pos.shape[1]
+    m = L ** 3 / n
+    h0 = hfact * m ** (1.0 / 3.0)
+    r = np.sqrt((pos * pos).sum(axis=0))
+    hi = 2.0 * h0
+    q = r / hi
+    w = np.where(q < 1.0, 1.0 - 1.5 * q * q + 0.75 * q ** 3, np.where(q < 2.0, 0.25 * (2.0 - q) ** 3, 0.0)) / (math.pi * hi ** 3)
+    u = E0 * w
+    return Workload(name or f"sedov{n_side}", pos, np.zeros((3, n)), np.full(n, m), u, np.full(n, h0),
+                    (-0.5 * L,) * 3, (0.5 * L,) * 3, (1, 1, 1), gamma, hfact, steps=steps, cfl=(cfl, cfl))
 
 
 def random_cloud(n: int, seed: int = DEFAULT_SEED, periodic: bool = True, clustered: bool = True,

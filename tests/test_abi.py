@@ -96,3 +96,20 @@ def test_workload_generators_are_deterministic_and_shaped():
     assert R.min() >= 2 and R.max() <= 10 and np.all(np.abs(d.pos[2]) <= 3 * 0.05 * R * (R / 2) ** 0.25 + 1e-12)
     u = W.splitmix_u01(1, np.arange(100000, dtype=np.uint64), 0)
     assert 0 <= u.min() and u.max() < 1 and abs(u.mean() - 0.5) < 0.01
+
+
+def test_sedov_workload_recipe():
+    """The Sedov-Taylor set-up: periodic HCP lattice (every site has 12 nearest neighbours at
+    one distance, to the few-per-cent stretch), unit density, injected energy sum m u = E0 to the lattice quadrature error."""
+    from paper_2503_09713_b200 import workloads as W
+    w = W.sedov(24)
+    assert w.n == 24 * 28 * 30 and w.cfl == (0.1, 0.1) and w.periodic == (1, 1, 1)
+    assert abs(w.mass.sum() / 1.2 ** 3 - 1.0) < 1e-12
+    assert abs((w.mass * w.u).sum() - 1.0) < 1e-3 and (w.u > 0).sum() < w.n // 4
+    L = 1.2
+    d = w.pos[:, :, None] - w.pos[:, None, :200]
+    d -= L * np.round(d / L)
+    r = np.sqrt((d * d).sum(axis=0))
+    r[r == 0] = 9.0
+    dx = L / 24
+    assert np.all(((r > 0.95 * dx) & (r < 1.05 * dx)).sum(axis=0) == 12) and r.min() > 0.95 * dx

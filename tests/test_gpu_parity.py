@@ -403,3 +403,22 @@ def test_density_size_classes_and_fallback_paths():
     sim = _sim(w)
     _stage_parity(w, sim)
     sim.close()
+
+
+def test_sedov_blast_stage_and_trajectory_parity():
+    """The paper's benchmark set-up (Sedov-Taylor blast on an HCP lattice):
+    u = 0 outside the injection region, so P = c_s = 0 there and the CFL minimum comes from the hot centre."""
+    w = W.sedov(20, cfl=0.1)
+    sim = _sim(w)
+    ev, f = _stage_parity(w, sim, expect_restarts=0)
+    s = O.State(w, "grid")
+    e0 = (w.mass * f["u"]).sum()
+    for _ in range(3):
+        dt_gpu = sim.step_leapfrog(want_dt=True)
+        assert dt_gpu == pytest.approx(s.step(), rel=1e-9)
+    g = _np(sim.get_fields())
+    assert np.max(np.abs(g["pos"] - s.pos)) < 1e-11 and np.max(np.abs(g["vel"] - s.vel)) < 1e-9 * np.abs(s.vel).max() + 1e-12
+    assert np.max(np.abs(g["u"] - s.u)) < 1e-9 * np.abs(s.u).max()
+    e1 = (w.mass * (0.5 * (g["vel"] ** 2).sum(axis=0) + g["u"])).sum()
+    assert abs(e1 / e0 - 1) < 1e-3
+    sim.close()
