@@ -64,40 +64,113 @@ __global__ void __launch_bounds__(256) k_group_fill(int64_t N, const uint32_t* _
     }
 }
 
-// bottom-up boxes: one thread per leaf; the second thread to reach a node merges its children and goes on.
-// A node whose two children are both leaves needs no flag: the left leaf's thread merges the pair directly and the
-// right leaf's thread retires at once (about half of all leaves, so half of the bottom-level atomics and fences).
-// Sibling records are read with L2 loads (ld.cg) issued after the flag atomic has returned, so only the release
-// side (record written -> fence -> flag) needs a fence.
-__global__ void __launch_bounds__(256) k_aabb(int64_t N, const double* __restrict__ x, const double* __restrict__ y,
-                                              const double* __restrict__ z, const double* __restrict__ h,
-                                              NodeRec* nodes, const int32_t* __restrict__ parent, uint32_t* visit) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    double lo[3] = {x[i], y[i], z[i]}, hi[3] = {lo[0], lo[1], lo[2]}, hm = h[i];
-    int32_t cur = (int32_t)i;
-    bool cur_leaf = true;
-    int32_t node = parent[N - 1 + i];
+// a3b: bottom-up boxes. A thread carrying a finished child box up the tree announces itself at the parent with an
+// atomic flag; the second arrival merges both children and goes on. Sibling records are read with L2 loads (ld.cg)
+// issued after the flag atomic has returned, so only the release side (record written -> fence -> flag) needs a fence.
+// Group-level boxes, kernel 1 of 2: one warp per leaf group (<= 32 consecutive leaves = one complete subtree).
+// Lane j holds leaf glo + j and looks after internal node glo + j if that node lies inside the subtree. The subtree
+// is evaluated bottom-up in rounds inside the warp: a node whose children are ready (a leaf always is) fetches their
+// boxes with shuffles and merges them. The bottom five levels of the tree thus need no flags, fences or dependent
+// L2 round trips, and the records are written once, coalesced.
+__global__ void __launch_bounds__(256) k_aabb_groups(int64_t N, const double* __restrict__ x, const double* __restrict__ y,
+                                                     const double* __restrict__ z, const double* __restrict__ h,
+                                                     NodeRec* nodes, const uint32_t* __restrict__ grp_lo,
+                                                     const DevScalars* sc) {
+    const unsigned lane = lane_id();
+    const uint32_t n_groups = sc->n_groups;
+    const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; g < n_groups; g += warps_total) {
+        const uint32_t glo = grp_lo[g], n = grp_lo[g + 1] - glo;
+        if (n < 2u) continue;                                 // a single leaf has no internal node
+        const uint32_t a = glo + (lane < n ? lane : 0u);
+        const double lx = x[a], ly = y[a], lz = z[a], lh = h[a];
+        const int64_t i = (int64_t)glo + lane;
+        bool mine = false, lleaf = false, rleaf = false;
+        int srcL = 0, srcR = 0;
+        if (lane < n && i < N - 1) {
+            const int32_t other = nodes[i].other, split = nodes[i].split;
+            const int64_t lo = min(i, (int64_t)other), hi = max(i, (int64_t)other);
+            mine = lo >= (int64_t)glo && hi < (int64_t)glo + n;
+            lleaf = (lo == split); rleaf = (hi == split + 1);
+            srcL = mine ? (int)(split - (int64_t)glo) : 0;
+            srcR = mine ? srcL + 1 : 0;
+        }
+        double b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0, b4 = 0.0, b5 = 0.0, b6 = 0.0;   // my node: lo xyz, hi xyz, hmax
+        bool done = !mine;
+        for (;;) {
+            const unsigned dm = __ballot_sync(0xffffffffu, done);
+            if (dm == 0xffffffffu) break;
+            const bool ok = !done && (lleaf || ((dm >> srcL) & 1u)) && (rleaf || ((dm >> srcR) & 1u));
+            // children: a leaf's box is its position, an internal child's box is that lane's node
+            const double Llx = __shfl_sync(0xffffffffu, lx, srcL), Lly = __shfl_sync(0xffffffffu, ly, srcL);
+            const double Llz = __shfl_sync(0xffffffffu, lz, srcL), Llh = __shfl_sync(0xffffffffu, lh, srcL);
+            const double Rlx = __shfl_sync(0xffffffffu, lx, srcR), Rly = __shfl_sync(0xffffffffu, ly, srcR);
+            const double Rlz = __shfl_sync(0xffffffffu, lz, srcR), Rlh = __shfl_sync(0xffffffffu, lh, srcR);
+            const double L0 = __shfl_sync(0xffffffffu, b0, srcL), L1 = __shfl_sync(0xffffffffu, b1, srcL);
+            const double L2 = __shfl_sync(0xffffffffu, b2, srcL), L3 = __shfl_sync(0xffffffffu, b3, srcL);
+            const double L4 = __shfl_sync(0xffffffffu, b4, srcL), L5 = __shfl_sync(0xffffffffu, b5, srcL);
+            const double L6 = __shfl_sync(0xffffffffu, b6, srcL);
+            const double R0 = __shfl_sync(0xffffffffu, b0, srcR), R1 = __shfl_sync(0xffffffffu, b1, srcR);
+            const double R2 = __shfl_sync(0xffffffffu, b2, srcR), R3 = __shfl_sync(0xffffffffu, b3, srcR);
+            const double R4 = __shfl_sync(0xffffffffu, b4, srcR), R5 = __shfl_sync(0xffffffffu, b5, srcR);
+            const double R6 = __shfl_sync(0xffffffffu, b6, srcR);
+            if (ok) {
+                b0 = fmin(lleaf ? Llx : L0, rleaf ? Rlx : R0); b1 = fmin(lleaf ? Lly : L1, rleaf ? Rly : R1);
+                b2 = fmin(lleaf ? Llz : L2, rleaf ? Rlz : R2); b3 = fmax(lleaf ? Llx : L3, rleaf ? Rlx : R3);
+                b4 = fmax(lleaf ? Lly : L4, rleaf ? Rly : R4); b5 = fmax(lleaf ? Llz : L5, rleaf ? Rlz : R5);
+                b6 = fmax(lleaf ? Llh : L6, rleaf ? Rlh : R6);
+                done = true;
+            }
+        }
+        if (mine) {
+            double* q = reinterpret_cast<double*>(nodes + i);
+            q[0] = b0; q[1] = b1; q[2] = b2; q[3] = b3; q[4] = b4; q[5] = b5; q[6] = b6;
+        }
+    }
+}
+
+// Group-level boxes, kernel 2 of 2: one thread per group carries the group's box (its root node's record, written
+// by kernel 1, or the single leaf) up the tree. A thread announces itself at the parent with an atomic flag; the
+// second arrival merges both children and goes on. Sibling records are read with L2 loads (ld.cg) issued after the
+// flag atomic has returned, so only the release side (record written -> fence -> flag) needs a fence.
+__global__ void __launch_bounds__(256) k_aabb_climb(int64_t N, const double* __restrict__ x, const double* __restrict__ y,
+                                                    const double* __restrict__ z, const double* __restrict__ h,
+                                                    NodeRec* nodes, const int32_t* __restrict__ parent, uint32_t* visit,
+                                                    const uint32_t* __restrict__ grp_lo, const DevScalars* sc) {
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= sc->n_groups) return;
+    const uint32_t glo = grp_lo[g], n = grp_lo[g + 1] - glo;
+    double lo[3], hi[3], hm;
+    int32_t cur;
+    bool cur_leaf = (n == 1u);
+    if (cur_leaf) {
+        cur = (int32_t)glo;
+        lo[0] = hi[0] = x[glo]; lo[1] = hi[1] = y[glo]; lo[2] = hi[2] = z[glo];
+        hm = h[glo];
+    } else {
+        // the group's root: the internal node whose range is the whole group (its index is one end of the range)
+        cur = (nodes[glo].other == (int32_t)(glo + n - 1u)) ? (int32_t)glo : (int32_t)(glo + n - 1u);
+        const double* p = reinterpret_cast<const double*>(nodes + cur);
+        lo[0] = p[0]; lo[1] = p[1]; lo[2] = p[2]; hi[0] = p[3]; hi[1] = p[4]; hi[2] = p[5]; hm = p[6];
+    }
+    int32_t node = cur_leaf ? parent[N - 1 + cur] : parent[cur];
+    bool wrote = false;                                        // records of kernel 1 are already visible
     while (node >= 0) {
-        const int32_t other = nodes[node].other, split = nodes[node].split;
-        const int32_t nlo = min(node, other), nhi = max(node, other);
+        if (wrote) __threadfence();                            // my record is visible before I announce myself
+        if (atomicAdd(&visit[node], 1u) == 0u) return;         // first arrival: the sibling's thread will carry on
+        asm volatile("" ::: "memory");                         // keep the sibling loads below the atomic
+        const int32_t oth = nodes[node].other, split = nodes[node].split;
+        const int32_t nlo = min(node, oth), nhi = max(node, oth);
         const bool lleaf = (nlo == split), rleaf = (nhi == split + 1);
         const bool i_am_left = (cur == split) && (cur_leaf == lleaf);
         const int32_t sib = i_am_left ? split + 1 : split;
         const bool sib_leaf = i_am_left ? rleaf : lleaf;
-        if (cur_leaf && sib_leaf) {
-            if (!i_am_left) return;                       // the left leaf's thread handles the pair
-        } else {
-            __threadfence();                              // my record is visible before I announce myself
-            if (atomicAdd(&visit[node], 1u) == 0u) return;    // first arrival: the sibling's thread will carry on
-            asm volatile("" ::: "memory");                // keep the sibling loads below the atomic in program order
-        }
         double slo[3], shi[3], shm;
         if (sib_leaf) {
             slo[0] = shi[0] = x[sib]; slo[1] = shi[1] = y[sib]; slo[2] = shi[2] = z[sib];
             shm = h[sib];
         } else {
-            const double* p = reinterpret_cast<const double*>(nodes + sib);   // read through L2: written by another SM
+            const double* p = reinterpret_cast<const double*>(nodes + sib);   // through L2: written by another SM
 #pragma unroll
             for (int k = 0; k < 3; ++k) { slo[k] = __ldcg(p + k); shi[k] = __ldcg(p + 3 + k); }
             shm = __ldcg(p + 6);
@@ -109,6 +182,7 @@ __global__ void __launch_bounds__(256) k_aabb(int64_t N, const double* __restric
 #pragma unroll
         for (int k = 0; k < 3; ++k) { __stcg(q + k, lo[k]); __stcg(q + 3 + k, hi[k]); }
         __stcg(q + 6, hm);
+        wrote = true;
         cur = node;
         cur_leaf = false;
         node = parent[node];
@@ -138,7 +212,11 @@ int launch_aabb(sph_ctx* c) {
     const int64_t N = c->N;
     if (N < 2) return SPH_OK;
     SPH_CUDA(c, cudaMemsetAsync(c->visit, 0, (size_t)(N - 1) * sizeof(uint32_t), c->stream));
-    k_aabb<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes, c->parent, c->visit);
+    // the group count of this tree is only known on the device: the climb grid is sized by its upper bound N
+    k_aabb_groups<<<148 * 16, 256, 0, c->stream>>>(N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes, c->grp_lo, c->d_sc);
+    k_aabb_climb<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes, c->parent, c->visit,
+                                                         c->grp_lo, c->d_sc);
+    c->launches++;
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
