@@ -57,7 +57,7 @@ struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 template <bool WRAP, bool UNIM, bool GLOB>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
                                             const uint32_t* __restrict__ cs,
-                                            const uint16_t* __restrict__ li, const uint32_t (&idx)[kRegChunks / 2],
+                                            const uint16_t* __restrict__ li, const uint32_t (&idx)[(kRegChunks + 1) / 2],
                                             int n, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
@@ -186,11 +186,11 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     }
     // the first 96 list entries of the octet's particle (two 16-bit indices per register), in flight together with
     // the staging copies
-    uint32_t idx[kRegChunks / 2];
+    uint32_t idx[(kRegChunks + 1) / 2];
 #pragma unroll
     for (int c = 0; c < kRegChunks; c += 2) {
         const int k0 = c * 8 + (int)sl, k1 = k0 + 8;
-        const uint32_t i0 = (k0 < n) ? (uint32_t)li[k0] : 0u, i1 = (k1 < n) ? (uint32_t)li[k1] : 0u;
+        const uint32_t i0 = (k0 < n) ? (uint32_t)li[k0] : 0u, i1 = (c + 1 < kRegChunks && k1 < n) ? (uint32_t)li[k1] : 0u;
         idx[c >> 1] = i0 | (i1 << 16);
     }
     cp_async_wait_all();
