@@ -127,8 +127,11 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
  * -> permute all fields into sorted order -> Karras radix tree (Table B2)
  * -> bottom-up AABB and max-h -> leaf groups (maximal nodes of <= 32 particles) -> traversal with
  * the group-group criterion and the object-object criterion with radius
- * R_kern chi max(h_a,h_b) -> neighbour cache by count, exclusive scan, fill (Alg. 5).
- * Synchronises the stream once (reads the neighbour total). */
+ * R_kern chi max(h_a,h_b) -> neighbour cache (the count / prefix / fill of Alg. 5, done per leaf
+ * group in one pass: hits are buffered on chip, counted, space is taken from a bump allocator, lists written).
+ * The cache is group-local: per group the array of candidate slots, per particle an ascending list of 16-bit
+ * indices into it; sph_get_neighbours converts to a CSR over sorted slots.
+ * Synchronises the stream once (reads the totals; repeats the pass with larger pools if one overflowed). */
 int sph_build_tree(sph_ctx* ctx);
 
 /* a5: Alg. 7 per particle over the cache, with the safeguard of reading A5b; rho from F1
