@@ -282,7 +282,7 @@ def main():
         flops = {"density": pairs * (FLOP_PER_PAIR_DENSITY_GATHER + FLOP_PER_PAIR_DENSITY_SWEEP * sweeps),
                  "forces": pairs * FLOP_PER_PAIR_FORCE,
                  "traverse": pairs * FLOP_PER_PAIR_TEST}
-        bytes_ = {"keys": 36 * n, "sort": 200 * n, "permute": 216 * n, "tree": 60 * n, "aabb": 148 * n,
+        bytes_ = {"keys": 36 * n, "sort": (8 + 24 * st.get("sort_passes", 8)) * n, "permute": 216 * n, "tree": 60 * n, "aabb": 148 * n,
                   "scan": 12 * n, "leapfrog": 272 * n}
         kernels = {}
         per_stage = {k: v for k, v in per_stage.items() if v > 0.0}

@@ -60,7 +60,8 @@ class Stats(C.Structure):
                 ("nbr_min", C.c_int32), ("nbr_max", C.c_int32), ("nbr_mean", C.c_double), ("h_iter_max", C.c_int32),
                 ("restarts", C.c_int32), ("steps", C.c_int64), ("kernel_launches", C.c_int64), ("dt", C.c_double),
                 ("t", C.c_double), ("bytes_allocated", C.c_int64), ("cand_max", C.c_int32), ("groups_fallback", C.c_int32),
-                ("chunks_shared", C.c_int32), ("share_chunk", C.c_int32)]
+                ("chunks_shared", C.c_int32), ("share_chunk", C.c_int32), ("sort_passes", C.c_int32),
+                ("sort_tie_max", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

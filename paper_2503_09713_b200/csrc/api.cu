@@ -143,6 +143,7 @@ static int cache_build(sph_ctx* c) {
             fprintf(stderr, "[sph] groups %u nc_max %u fallback %u nbr_min %u nbr_max %u lists %llu candidates %llu chunk %u shared %u overflow %u\n",
                     s.n_groups, s.nc_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.cslot_cursor, c->last_chunk,
                     s.n_chunks_shared, s.n_chunks_overflow);
+        c->sort_p0 = (s.tie_max <= 64u && !getenv("SPH_FULL_SORT")) ? 3 : 0;   // next sort: prefix mode if ties stay short
         if (c->last_chunk > 1) {
             const uint64_t chunks = ((uint64_t)s.n_groups + c->last_chunk - 1) / c->last_chunk;
             if ((uint64_t)s.n_chunks_shared * 10 < chunks * 8 || (uint64_t)s.n_chunks_overflow * 50 > chunks)
@@ -540,6 +541,7 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->kernel_launches = c->launches; out->dt = s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
     out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
     out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
+    out->sort_passes = c->last_sort_passes; out->sort_tie_max = (int32_t)s.tie_max;
     return SPH_OK;
 }
 

@@ -65,6 +65,7 @@ struct DevScalars {
     unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
     unsigned int n_chunks_shared;    // traversal chunks that shared one walk / whose shared walk overflowed
     unsigned int n_chunks_overflow;
+    unsigned int tie_max;            // longest run of keys equal in their top 40 bits (sort prefix mode)
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
 };
@@ -131,6 +132,8 @@ struct sph_ctx {
     double t = 0.0;
     int64_t launches = 0;
     bool have_cfl_dt = false;
+    int last_sort_passes = 8;
+    int sort_p0 = 0;                    // first radix pass: 0 = all eight passes, 3 = prefix mode (top 40 bits + repair)
     bool share_disabled = false;        // traversal: shared walks switched off (too few chunks could share)
     uint32_t last_chunk = 1;
     bool uniform_mass = false;          // all particle masses equal (density kernel variant)

@@ -3,6 +3,8 @@
 // are resolved with a decoupled look-back over single-word (flag|count) status entries; ranking inside a tile
 // uses warp-level __match_any_sync multisplit. Replaces the paper's bitonic sort, which it
 // says dominates the tree build. HBM-bound: 8 B + 8 x 24 B = 200 B per particle.
+#include <utility>
+
 #include "common.cuh"
 
 namespace sph {
@@ -10,6 +12,8 @@ namespace sph {
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kPasses = 8;
+constexpr int kPrefixPass = 3;                   // prefix mode sorts on digits 3..7 = bits 24..63 (40 bits)
+constexpr int kPrefixShift = kPrefixPass * 8;
 constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kItems = 16;                       // keys per thread
@@ -18,7 +22,7 @@ constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 
 
 // ---- kernel 1: histograms of all 8 digits in one read of the keys ----
 __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ key, int64_t N,
-                                                   uint32_t* __restrict__ ghist) {
+                                                   uint32_t* __restrict__ ghist, int p0) {
     __shared__ uint32_t sh[kPasses][kRadix];
     for (int i = threadIdx.x; i < kPasses * kRadix; i += blockDim.x) (&sh[0][0])[i] = 0;
     __syncthreads();
@@ -32,6 +36,7 @@ __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ 
             uint64_t k = key[i];
 #pragma unroll
             for (int p = 0; p < kPasses; ++p) {
+                if (p < p0) continue;                            // digits below the first pass are not sorted on
                 unsigned d = (unsigned)(k >> (p * kRadixBits)) & (kRadix - 1);
                 unsigned m = __match_any_sync(act, d);           // warp-aggregated histogram update
                 if (lane == (unsigned)(__ffs(m) - 1)) atomicAdd(&sh[p][d], __popc(m));
@@ -46,7 +51,8 @@ __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ 
 }
 
 // ---- kernel 2: exclusive scan of each digit histogram -> global digit bases ----
-__global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ ghist) {
+__global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ ghist, DevScalars* sc) {
+    if (threadIdx.x == 0) sc->tie_max = 0u;
     __shared__ uint32_t wsum[kRadix / 32];
     const unsigned d = threadIdx.x, lane = lane_id(), w = d >> 5;
     for (int p = 0; p < kPasses; ++p) {
@@ -190,6 +196,32 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __
     }
 }
 
+// ---- kernel 4: tie repair / census for the prefix mode ----
+// In prefix mode only the digits above bit `shift` are sorted on (stable LSD passes), which leaves keys that share
+// those bits in their previous order. The thread at the head of each run of equal prefixes insertion-sorts the run
+// by the full key (stable, so equal keys keep their previous order): the result is exactly the stable sort by the
+// full key. Runs are rare and short when the prefix resolves the particles (40 of 63 bits: cells of 2^-13.3 of the
+// box per axis); the longest run is recorded so that the host falls back to all eight passes when it is not.
+__global__ void __launch_bounds__(256) k_sort_repair(int64_t N, uint64_t* __restrict__ key, uint32_t* __restrict__ val,
+                                                     int shift, DevScalars* sc) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint64_t p = key[i] >> shift;
+    if (i > 0 && (key[i - 1] >> shift) == p) return;          // not the head of a run
+    int64_t e = i + 1;
+    while (e < N && (key[e] >> shift) == p) ++e;
+    if (e - i < 2) return;
+    atomicMax(&sc->tie_max, (unsigned int)min(e - i, (int64_t)0x7fffffff));
+    for (int64_t a = i + 1; a < e; ++a) {
+        const uint64_t kk = key[a];
+        const uint32_t vv = val[a];
+        int64_t b = a - 1;
+        while (b >= i && key[b] > kk) { key[b + 1] = key[b]; val[b + 1] = val[b]; --b; }
+        key[b + 1] = kk;
+        val[b + 1] = vv;
+    }
+}
+
 int sort_scratch_bytes(int64_t N, int64_t* tiles, size_t* status_bytes) {
     *tiles = (N + kTile - 1) / kTile;
     *status_bytes = (size_t)kPasses * (size_t)(*tiles) * kRadix * sizeof(uint32_t);
@@ -208,12 +240,16 @@ int launch_sort(sph_ctx* c) {
     SPH_CUDA(c, cudaMemsetAsync(c->sort_status, 0, kPasses * status_per_pass * sizeof(uint32_t), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(c->sort_counters, 0, kPasses * sizeof(uint32_t), c->stream));
     unsigned hb = (unsigned)min((int64_t)148 * 8, (N + 255) / 256);
-    k_sort_hist<<<hb, 256, 0, c->stream>>>(c->key, N, c->sort_hist);
-    k_sort_bases<<<1, kRadix, 0, c->stream>>>(c->sort_hist);
+    // Prefix mode: sort on the top 40 bits only (five passes) and repair the rare runs of equal prefixes; chosen by
+    // the host from the longest run seen in the previous sort (api.cu), all eight passes otherwise.
+    const int p0 = c->sort_p0;
+    c->last_sort_passes = kPasses - p0;
+    k_sort_hist<<<hb, 256, 0, c->stream>>>(c->key, N, c->sort_hist, p0);
+    k_sort_bases<<<1, kRadix, 0, c->stream>>>(c->sort_hist, c->d_sc);
     c->launches += 2;
     uint64_t *kin = c->key, *kout = c->key_alt;
     uint32_t *vin = c->val, *vout = c->val_alt;
-    for (int p = 0; p < kPasses; ++p) {
+    for (int p = p0; p < kPasses; ++p) {
         k_onesweep<<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
             kin, vin, kout, vout, N, p * kRadixBits, c->sort_hist + p * kRadix,
             c->sort_status + p * status_per_pass, c->sort_counters + p);
@@ -221,8 +257,13 @@ int launch_sort(sph_ctx* c) {
         uint64_t* tk = kin; kin = kout; kout = tk;
         uint32_t* tv = vin; vin = vout; vout = tv;
     }
+    if ((kPasses - p0) & 1) {   // odd number of passes: the result is in the other pair of buffers
+        std::swap(c->key, c->key_alt);
+        std::swap(c->val, c->val_alt);
+    }
+    k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, c->d_sc);
+    c->launches++;
     SPH_CUDA(c, cudaGetLastError());
-    // kPasses is even: the result is back in c->key / c->val
     return SPH_OK;
 }
 

@@ -422,3 +422,58 @@ def test_sedov_blast_stage_and_trajectory_parity():
     e1 = (w.mass * (0.5 * (g["vel"] ** 2).sum(axis=0) + g["u"])).sum()
     assert abs(e1 / e0 - 1) < 1e-3
     sim.close()
+
+
+def _check_sorted_state(sim, pos, box, prev_perm=None):
+    """Keys bit-exact against the oracle's keys of `pos` sorted; permutation valid; equal keys in the order of the
+    slots they came from (stability), which is the original index when prev_perm is None."""
+    key = O.morton_keys(pos, box)
+    gkey, gperm = sim.get_keys_perm()
+    assert np.array_equal(gkey, np.sort(key)) and np.array_equal(key[gperm], gkey)
+    assert np.array_equal(np.sort(gperm), np.arange(pos.shape[1]))
+    came_from = gperm.astype(np.int64)
+    if prev_perm is not None:
+        inv = np.empty(prev_perm.size, np.int64)
+        inv[prev_perm] = np.arange(prev_perm.size)
+        came_from = inv[gperm]
+    same = gkey[1:] == gkey[:-1]
+    assert np.all(came_from[1:][same] > came_from[:-1][same])
+    return gperm
+
+
+@pytest.mark.parametrize("cluster", [24, 200], ids=["short_runs_prefix_mode", "long_runs_full_sort"])
+def test_sort_prefix_mode_and_tie_repair(cluster):
+    """From the second build on the sort uses five passes over the top 40 key bits plus a repair of the runs that
+    share them, if the previous sort saw only short runs (<= 64), else all eight passes. Clusters of particles
+    inside one 2^-14 cell make such runs; both modes must give the stable sort by the full key."""
+    from paper_2503_09713_b200 import binding as B
+    n, ncl = 6000, 12
+    w = W.random_cloud(n, seed=31, periodic=False, clustered=False)
+    rng = np.random.default_rng(cluster)
+
+    def clustered(pos):
+        pos = pos.copy()
+        for c in range(ncl):
+            sel = slice(c * cluster, (c + 1) * cluster)
+            pos[:, sel] = pos[:, sel.start:sel.start + 1] + 1e-6 * rng.random((3, cluster))
+        pos[:, ncl * cluster:ncl * cluster + 4] = pos[:, ncl * cluster:ncl * cluster + 1]    # identical keys too
+        return np.clip(pos, 0.0, np.nextafter(1.0, 0.0))
+
+    w.pos = clustered(w.pos)
+    box, p = O.workload_box_params(w)
+    sim = B.Sim.from_workload(w, white_step=False)
+    sim.build_tree()
+    st = sim.stats()
+    assert st["sort_passes"] == 8 and st["sort_tie_max"] >= cluster
+    perm0 = _check_sorted_state(sim, w.pos, box)
+    # new positions: every particle moves, clusters are re-drawn; the next sort starts from the previous order
+    pos1 = clustered(np.clip(w.pos + 0.01 * (rng.random((3, n)) - 0.5), 0.0, np.nextafter(1.0, 0.0)))
+    sim.set_fields(pos=pos1)
+    sim.build_tree()
+    st = sim.stats()
+    assert st["sort_passes"] == (5 if cluster <= 64 else 8)
+    _check_sorted_state(sim, pos1, box, prev_perm=perm0)
+    oo, oi = O.neighbours(pos1[:, sim.get_keys_perm()[1]], w.h0[sim.get_keys_perm()[1]], box, p.chi, "grid")
+    go, gi = sim.get_neighbours()
+    assert np.array_equal(go, oo)
+    sim.close()
