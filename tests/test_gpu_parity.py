@@ -477,3 +477,32 @@ def test_sort_prefix_mode_and_tie_repair(cluster):
     go, gi = sim.get_neighbours()
     assert np.array_equal(go, oo)
     sim.close()
+
+
+def test_long_run_conservation_and_reproducibility():
+    """40 leapfrog steps of a perturbed 32^3 cube (prefix-mode sort, cache pools reused and regrown, dt from the
+    device): total energy drifts by less than 1e-5 (PAPER.md:208 quotes 1e-6 for its runs), momentum stays at
+    round-off, and a second run of the same input gives bitwise identical fields (no result depends on the order in
+    which warps allocate cache space or arrive at tree nodes)."""
+    w = W.cube(32, jitter=0.1, vel_amp=0.05, seed=17)
+
+    def run():
+        sim = _sim(w)
+        f0 = _np(sim.get_fields(("vel", "u")))
+        for _ in range(40):
+            sim.step_leapfrog()
+        f = _np(sim.get_fields())
+        st = sim.stats()
+        sim.close()
+        return f0, f, st
+
+    f0, f, st = run()
+    assert st["steps"] == 40 and st["sort_passes"] == 5 and st["restarts"] == 0
+    e0 = (w.mass * (0.5 * (f0["vel"] ** 2).sum(axis=0) + f0["u"])).sum()
+    e1 = (w.mass * (0.5 * (f["vel"] ** 2).sum(axis=0) + f["u"])).sum()
+    assert abs(e1 / e0 - 1) < 1e-5
+    assert np.all(np.abs((w.mass * f["vel"]).sum(axis=1) - (w.mass * f0["vel"]).sum(axis=1)) < 1e-14)
+    assert np.all(np.isfinite(f["acc"])) and f["rho"].min() > 0.8 and f["rho"].max() < 1.25
+    _, g, _ = run()
+    for k in f:
+        assert np.array_equal(f[k], g[k]), k
