@@ -73,6 +73,13 @@ typedef struct {
   double cs0, r0, q;    /* locally isothermal EOS; R = cylindrical radius about centre[]                     */
   double GM, soft;      /* fixed point mass a_ext = -GM d / (|d|^2 + soft^2)^(3/2); GM = 0 disables          */
   double centre[3];
+  /* Leapfrog corrector check and re-cycle, G6-G7, and CFL multiplier, G9-G10
+   * (PAPER.md:1337-1345); readings A15, A16. */
+  double eps_v;         /* 0 (off; the paper uses 1e-2): after the corrector, while max|dv| / rms|v| >= eps_v the
+                           acceleration is recalculated with v* <- v^{n+1} and the correction applied again   */
+  double lambda_stiff;  /* 2.0  stiffness of the CFL multiplier relaxation (value not given in the paper)        */
+  int32_t max_recycle;  /* 10   cap on re-cycles per step                                                        */
+  int32_t reserved2;
 } sph_params;
 
 /* Device-memory hooks so that the host framework (PyTorch's caching allocator) owns device memory.
@@ -107,6 +114,9 @@ typedef struct {
   int32_t share_chunk;     /* groups per chunk used by the last pass (1 or 4)                             */
   int32_t sort_passes;     /* radix passes of the last sort: 8, or 5 in prefix mode (top 40 bits + tie repair) */
   int32_t sort_tie_max;    /* longest run of keys equal in their top 40 bits seen by the last sort         */
+  int32_t recycles;        /* corrector re-cycles of the last step (eps_v > 0)                              */
+  int32_t reserved;
+  double cfl_mult;         /* CFL multiplier lambda_CFL applied to the next internal dt                     */
 } sph_stats;
 
 void sph_default_params(sph_params* p);

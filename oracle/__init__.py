@@ -37,7 +37,8 @@ class Params(C.Structure):
                 ("c_cour", C.c_double), ("c_force", C.c_double), ("max_h_iter", C.c_int32),
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("newton_literal", C.c_int32),
                 ("cs0", C.c_double), ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
-                ("centre", C.c_double * 3)]
+                ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
+                ("max_recycle", C.c_int32), ("pad_", C.c_int32)]
 
 
 def make_box(lo, hi, periodic) -> Box:
@@ -46,11 +47,12 @@ def make_box(lo, hi, periodic) -> Box:
 
 def make_params(gamma=5.0 / 3.0, hfact=1.2, chi=1.1, lam=1.2, eps_h=1e-6, alpha_av=1.0, beta_av=2.0, beta_u=1.0,
                 c_cour=0.3, c_force=0.25, max_h_iter=50, max_restarts=50, eos_isothermal=None, point_mass=None,
-                newton_literal=0) -> Params:
+                newton_literal=0, eps_v=0.0, lambda_stiff=2.0, max_recycle=10) -> Params:
     p = Params()
     p.hfact, p.gamma, p.chi, p.lam, p.eps_h = hfact, gamma, chi, lam, eps_h
     p.alpha_av, p.beta_av, p.beta_u, p.c_cour, p.c_force = alpha_av, beta_av, beta_u, c_cour, c_force
     p.max_h_iter, p.max_restarts, p.newton_literal = max_h_iter, max_restarts, newton_literal
+    p.eps_v, p.lambda_stiff, p.max_recycle = eps_v, lambda_stiff, max_recycle
     p.eos = 0
     if eos_isothermal is not None:
         p.eos = 1
@@ -66,6 +68,8 @@ def workload_box_params(w, **kw):
     cfl = getattr(w, "cfl", None)
     if cfl is not None:
         kw = dict(dict(c_cour=cfl[0], c_force=cfl[1]), **kw)
+    if getattr(w, "eps_v", None):
+        kw = dict(dict(eps_v=w.eps_v), **kw)
     return (make_box(w.box_lo, w.box_hi, w.periodic),
             make_params(gamma=w.gamma, hfact=w.hfact, eos_isothermal=w.eos_isothermal, point_mass=w.point_mass, **kw))
 
@@ -90,6 +94,7 @@ def lib():
         _lib.orc_forces.restype = C.c_double
         _lib.orc_evaluate.restype = C.c_int32
         _lib.orc_step.restype = C.c_int32
+        _lib.orc_step2.restype = C.c_int32
     return _lib
 
 
@@ -236,17 +241,22 @@ class State:
         self.t = 0.0
 
     def step(self, dt=None):
+        """One leapfrog step (with the corrector re-cycle and CFL multiplier if the parameters set eps_v > 0)."""
         dt = self.dt if dt is None or dt <= 0 else dt
         n = self.pos.shape[1]
         dtn = C.c_double()
-        rc = lib().orc_step(C.c_int64(n), _p(self.pos, np.float64), _p(self.vel, np.float64), _p(self.m, np.float64),
-                            _p(self.u, np.float64), _p(self.h, np.float64), _p(self.acc, np.float64),
-                            _p(self.dudt, np.float64), C.byref(self.box), C.byref(self.p),
-                            C.c_int32(0 if self.mode == "brute" else 1), C.c_double(dt), _p(self.rho, np.float64),
-                            _p(self.omega, np.float64), C.byref(dtn))
+        mult = C.c_double(getattr(self, "cfl_mult", 1.0))
+        nrec = C.c_int32()
+        rc = lib().orc_step2(C.c_int64(n), _p(self.pos, np.float64), _p(self.vel, np.float64), _p(self.m, np.float64),
+                             _p(self.u, np.float64), _p(self.h, np.float64), _p(self.acc, np.float64),
+                             _p(self.dudt, np.float64), C.byref(self.box), C.byref(self.p),
+                             C.c_int32(0 if self.mode == "brute" else 1), C.c_double(dt), _p(self.rho, np.float64),
+                             _p(self.omega, np.float64), C.byref(dtn), C.byref(mult), C.byref(nrec))
         if rc < 0:
             raise RuntimeError("oracle: " + _ERR.get(rc, str(rc)))
         self.restarts = int(rc)
+        self.recycles = int(nrec.value)
+        self.cfl_mult = float(mult.value)
         self.t += dt
         self.dt = dtn.value
         return dt

@@ -50,6 +50,10 @@ struct orc_params {
     double cs0, r0, q;
     double GM, soft;   // fixed softened point mass (BASELINE config 3); GM = 0 disables
     double centre[3];
+    double eps_v;        // leapfrog corrector check G7: 1e-2 in the paper; 0 disables (reading A15)
+    double lambda_stiff; // stiffness of the CFL multiplier G10; value not given, reading A16
+    int32_t max_recycle; // cap on corrector re-cycles per step
+    int32_t pad_;
 };
 
 }  // extern "C"
@@ -486,11 +490,12 @@ double orc_forces(int64_t N, const double* pos, const double* vel, const double*
 // forces. h is in/out (h^n in, converged h out). mode 0 = brute-force neighbour search, 1 = cell grid.
 // Returns restarts >= 0, or -1 (h iteration cap), -2 (restart cap). If offs_out/idx_out are non-null and
 // cap suffices they receive the final cache.
-int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
-                     double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
-                     double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out) {
-    std::vector<uint64_t> offs(N + 1);
-    std::vector<uint32_t> idx;
+static int32_t evaluate_impl(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
+                             double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
+                             double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out,
+                             std::vector<uint64_t>& offs, std::vector<uint32_t>& idx) {
+    offs.assign(N + 1, 0);
+    idx.clear();
     std::vector<double> hn(h, h + N), hnew(N);
     int32_t restarts = 0;
     for (;;) {
@@ -512,12 +517,29 @@ int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const doub
     return restarts;
 }
 
+int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
+                     double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
+                     double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out) {
+    std::vector<uint64_t> offs;
+    std::vector<uint32_t> idx;
+    return evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, dt_out, n_neigh_out, offs, idx);
+}
+
 // ---- O10: one leapfrog KDK step (G1-G5; order of Fig. G1; u integrated
 // like v, reading A13). State in/out: pos, vel, u, h, acc, dudt (a^n, du/dt^n on entry; ^{n+1} on exit).
 // Returns restarts or a negative error like orc_evaluate; dt_next receives the CFL dt for the next step (A14).
-int32_t orc_step(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
-                 double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
-                 double* omega, double* dt_next) {
+//
+// Corrector check and re-cycle (G6-G7), only if p->eps_v > 0. Reading A15: G7 as printed divides
+// max|dv| by the rms of dv itself, which is >= 1 for any data and can never be below eps_v = 1e-2; the check is
+// taken as in Phantom (which the paper says it follows): err = max_i |dv_i| / sqrt((1/N) sum_j |v_j^{n+1}|^2), 0 if
+// all velocities vanish. While err >= eps_v (at most max_recycle times): the acceleration is recalculated with
+// v* <- v^{n+1} (and u* <- u^{n+1}) on the same positions, h, rho, Omega and neighbour cache, and the correction
+// dv = dt/2 (a_new - a_previous) is applied again. CFL multiplier (G9-G10): *cfl_mult is
+// halved after a step that re-cycled, else relaxed by (1 + stiff * mult) / (1 + stiff) (reading A16: lambda_stiff is
+// not given in the paper; it is a parameter); dt_next = mult * G8, as both terms of G8 are linear in the C's.
+int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                  double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                  double* omega, double* dt_next, double* cfl_mult, int32_t* n_recycle) {
     std::vector<double> a_old(acc, acc + 3 * N), du_old(dudt, dudt + N);
     for (int c = 0; c < 3; ++c) {
         double L = box->hi[c] - box->lo[c];
@@ -537,11 +559,51 @@ int32_t orc_step(int64_t N, double* pos, double* vel, const double* m, double* u
         double uh = u[i] + 0.5 * dt * du_old[i];
         u[i] = uh + 0.5 * dt * du_old[i];
     }
-    int32_t rc = orc_evaluate(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, dt_next, nullptr);   // G4
+    std::vector<uint64_t> offs;
+    std::vector<uint32_t> idx;
+    double dt_raw = 0.0;
+    int32_t rc = evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, &dt_raw, nullptr, offs, idx);   // G4
     if (rc < 0) return rc;
-    for (int64_t i = 0; i < 3 * N; ++i) vel[i] = vel[i] + 0.5 * dt * (acc[i] - a_old[i]);                     // G5
-    for (int64_t i = 0; i < N; ++i) u[i] = u[i] + 0.5 * dt * (dudt[i] - du_old[i]);
+    int32_t recycles = 0;
+    for (;;) {
+        double dvmax2 = 0.0, v2sum = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            double d2 = 0.0, v2 = 0.0;
+            for (int c = 0; c < 3; ++c) {
+                const double dv = 0.5 * dt * (acc[c * N + i] - a_old[c * N + i]);                                 // G5, G6
+                vel[c * N + i] = vel[c * N + i] + dv;
+                d2 += dv * dv;
+                v2 += vel[c * N + i] * vel[c * N + i];
+            }
+            dvmax2 = std::max(dvmax2, d2);
+            v2sum += v2;
+            u[i] = u[i] + 0.5 * dt * (dudt[i] - du_old[i]);
+        }
+        if (!(p->eps_v > 0.0) || recycles >= p->max_recycle) break;
+        const double vrms = std::sqrt(v2sum / (double)N);
+        const double err = vrms > 0.0 ? std::sqrt(dvmax2) / vrms : 0.0;                                           // G7 (A15)
+        if (err < p->eps_v) break;
+        ++recycles;
+        a_old.assign(acc, acc + 3 * N);
+        du_old.assign(dudt, dudt + N);
+        dt_raw = orc_forces(N, pos, vel, m, h, rho, omega, u, offs.data(), idx.data(), box, p, acc, dudt);
+    }
+    double mult = cfl_mult ? *cfl_mult : 1.0;
+    if (p->eps_v > 0.0) {
+        mult = recycles > 0 ? 0.5 * mult : (1.0 + p->lambda_stiff * mult) / (1.0 + p->lambda_stiff);              // G9-G10
+        if (cfl_mult) *cfl_mult = mult;
+    }
+    if (dt_next) *dt_next = mult * dt_raw;
+    if (n_recycle) *n_recycle = recycles;
     return rc;
+}
+
+int32_t orc_step(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                 double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                 double* omega, double* dt_next) {
+    orc_params q = *p;
+    q.eps_v = 0.0;                                   // the plain step of G1-G5: no corrector check
+    return orc_step2(N, pos, vel, m, u, h, acc, dudt, box, &q, mode, dt, rho, omega, dt_next, nullptr, nullptr);
 }
 
 }  // extern "C"

@@ -42,7 +42,8 @@ class Params(C.Structure):
                 ("c_cour", C.c_double), ("c_force", C.c_double), ("max_h_iter", C.c_int32),
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("reserved", C.c_int32), ("cs0", C.c_double),
                 ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
-                ("centre", C.c_double * 3)]
+                ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
+                ("max_recycle", C.c_int32), ("reserved2", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -61,7 +62,7 @@ class Stats(C.Structure):
                 ("restarts", C.c_int32), ("steps", C.c_int64), ("kernel_launches", C.c_int64), ("dt", C.c_double),
                 ("t", C.c_double), ("bytes_allocated", C.c_int64), ("cand_max", C.c_int32), ("groups_fallback", C.c_int32),
                 ("chunks_shared", C.c_int32), ("share_chunk", C.c_int32), ("sort_passes", C.c_int32),
-                ("sort_tie_max", C.c_int32)]
+                ("sort_tie_max", C.c_int32), ("recycles", C.c_int32), ("reserved", C.c_int32), ("cfl_mult", C.c_double)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -122,6 +123,8 @@ def params_for(w, **kw) -> Params:
         extra.update(GM=w.point_mass[0], soft=w.point_mass[1], centre=w.point_mass[2])
     if getattr(w, "cfl", None) is not None:
         extra.update(c_cour=w.cfl[0], c_force=w.cfl[1])
+    if getattr(w, "eps_v", None):
+        extra.update(eps_v=w.eps_v)
     extra.update(kw)
     return default_params(**extra)
 

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/sph_b200.h: context, memory, call-order state machine, step orchestration,
 // getters/setters and per-stage CUDA-event timers. All arithmetic of the hot path lives in the kernels of the
 // sibling .cu files; there is no CPU fallback anywhere in this library.
+#include <math.h>
 #include <stdarg.h>
 #include <stdlib.h>
 #include <string.h>
@@ -184,6 +185,7 @@ void sph_default_params(sph_params* p) {
     p->alpha_av = 1.0; p->beta_av = 2.0; p->beta_u = 1.0; p->c_cour = 0.3; p->c_force = 0.25;
     p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0;
     p->cs0 = 1.0; p->r0 = 1.0; p->q = 0.0; p->GM = 0.0; p->soft = 0.0;
+    p->eps_v = 0.0; p->lambda_stiff = 2.0; p->max_recycle = 10;
 }
 
 const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
@@ -246,6 +248,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
     SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
     SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
+    SPH_TRY(dalloc(c, &c->corr_part, 2 * (size_t)div_up(N, 256) + 2));
     // cache pools start empty: the first traversal only counts, then they are sized from its totals
     c->scan_tiles = scan_scratch_tiles(N);
     SPH_TRY(dalloc(c, &c->scan_status, (size_t)c->scan_tiles));
@@ -360,7 +363,25 @@ int sph_step_leapfrog(sph_ctx* c, double dt, double* dt_used) {
     SPH_TRY(sph_build_tree(c));
     SPH_TRY(sph_compute_density(c));
     SPH_TRY(forces_eval(c));
-    { StageTimer t(c, ST_LEAPFROG); SPH_TRY(launch_correct(c)); }
+    const bool check = c->p.eps_v > 0.0;
+    { StageTimer t(c, ST_LEAPFROG); SPH_TRY(launch_correct(c, check)); }
+    c->recycles_last = 0;
+    if (check) {
+        // G6-G7 with reading A15: err = max|dv| / rms|v^{n+1}|; while it is not below eps_v, recalculate the
+        // acceleration with v* <- v^{n+1} (same positions, h, rho, Omega, cache) and apply the correction again
+        for (;;) {
+            SPH_TRY(read_scalars(c));
+            const double vrms = sqrt(c->h_sc->corr_v2sum / (double)c->N);
+            const double err = vrms > 0.0 ? sqrt(c->h_sc->corr_dvmax2) / vrms : 0.0;
+            if (err < c->p.eps_v || c->recycles_last >= c->p.max_recycle) break;
+            c->recycles_last++;
+            SPH_TRY(forces_eval(c));
+            { StageTimer t(c, ST_LEAPFROG); SPH_TRY(launch_correct(c, true)); }
+        }
+        // G9-G10: halve the multiplier after a step that re-cycled, relax it towards 1 otherwise
+        c->cfl_mult = c->recycles_last > 0 ? 0.5 * c->cfl_mult
+                                            : (1.0 + c->p.lambda_stiff * c->cfl_mult) / (1.0 + c->p.lambda_stiff);
+    }
     c->steps++;
     if (dt_used) {
         SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d_dtstep, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -538,10 +559,11 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->nbr_min = (int32_t)s.nbr_min; out->nbr_max = (int32_t)s.nbr_max;
     out->nbr_mean = c->N ? (double)c->n_neigh / (double)c->N : 0.0;
     out->h_iter_max = (int32_t)s.h_iter_max; out->restarts = c->restarts_last; out->steps = c->steps;
-    out->kernel_launches = c->launches; out->dt = s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
+    out->kernel_launches = c->launches; out->dt = c->cfl_mult * s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
     out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
     out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
     out->sort_passes = c->last_sort_passes; out->sort_tie_max = (int32_t)s.tie_max;
+    out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult;
     return SPH_OK;
 }
 

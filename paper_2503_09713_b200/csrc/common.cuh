@@ -65,6 +65,7 @@ struct DevScalars {
     unsigned int n_cand_overflow;    // groups with more than 65535 candidates (16-bit local index overflow)
     unsigned int n_chunks_shared;    // traversal chunks that shared one walk / whose shared walk overflowed
     unsigned int n_chunks_overflow;
+    double corr_dvmax2, corr_v2sum;  // corrector check G7: max |dv|^2, sum |v|^2 (reading A15)
     unsigned int tie_max;            // longest run of keys equal in their top 40 bits (sort prefix mode)
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
@@ -132,6 +133,9 @@ struct sph_ctx {
     double t = 0.0;
     int64_t launches = 0;
     bool have_cfl_dt = false;
+    double* corr_part = nullptr;        // per-block partials of the corrector check (2 x blocks)
+    double cfl_mult = 1.0;              // CFL multiplier lambda_CFL (G9-G10)
+    int recycles_last = 0;              // corrector re-cycles of the last step
     int last_sort_passes = 8;
     int sort_p0 = 0;                    // first radix pass: 0 = all eight passes, 3 = prefix mode (top 40 bits + repair)
     bool share_disabled = false;        // traversal: shared walks switched off (too few chunks could share)
@@ -176,7 +180,7 @@ int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n
 int launch_density(sph_ctx* c);                                // density.cu
 int launch_forces(sph_ctx* c);                                 // forces.cu
 int launch_predict(sph_ctx* c);                                // leapfrog.cu
-int launch_correct(sph_ctx* c);                                // leapfrog.cu
+int launch_correct(sph_ctx* c, bool with_check);                           // leapfrog.cu
 int launch_hmax(sph_ctx* c);                                   // leapfrog.cu  max h^n -> d_sc->h_max
 int launch_adopt_acc(sph_ctx* c);                              // leapfrog.cu  a^n <- a^{n+1} (white step)
 int launch_set_dt(sph_ctx* c, double user_dt);                 // leapfrog.cu  device dt for predictor/corrector; t += dt

@@ -43,17 +43,55 @@ __global__ void __launch_bounds__(256) k_predict(int64_t N, Fields f, WrapBox wb
 }
 
 // G5: v = v* + dt/2 (a_new - a_old); then a_old <- a_new (same for u)
+// G5: v = v* + dt/2 (a_new - a_old); then a_old <- a_new (same for u). With ERR the kernel also reduces, per block
+// and in a fixed order, the two quantities of the corrector check G6-G7 (reading A15):
+// max |dv|^2 and sum |v^{n+1}|^2.
+template <bool ERR>
 __global__ void __launch_bounds__(256) k_correct(int64_t N, Fields f, const double* __restrict__ nax,
                                                  const double* __restrict__ nay, const double* __restrict__ naz,
-                                                 const double* __restrict__ ndu, const double* __restrict__ dtp) {
+                                                 const double* __restrict__ ndu, const double* __restrict__ dtp,
+                                                 double* __restrict__ part_max, double* __restrict__ part_sum) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const double hdt = 0.5 * *dtp;
-    double a;
-    a = nax[i]; f.vx[i] = f.vx[i] + hdt * (a - f.ax[i]); f.ax[i] = a;
-    a = nay[i]; f.vy[i] = f.vy[i] + hdt * (a - f.ay[i]); f.ay[i] = a;
-    a = naz[i]; f.vz[i] = f.vz[i] + hdt * (a - f.az[i]); f.az[i] = a;
-    a = ndu[i]; f.u[i] = f.u[i] + hdt * (a - f.du[i]); f.du[i] = a;
+    double d2 = 0.0, v2 = 0.0;
+    if (i < N) {
+        const double hdt = 0.5 * *dtp;
+        double a, dv, v;
+        a = nax[i]; dv = hdt * (a - f.ax[i]); v = f.vx[i] + dv; f.vx[i] = v; f.ax[i] = a; d2 = dv * dv; v2 = v * v;
+        a = nay[i]; dv = hdt * (a - f.ay[i]); v = f.vy[i] + dv; f.vy[i] = v; f.ay[i] = a; d2 += dv * dv; v2 += v * v;
+        a = naz[i]; dv = hdt * (a - f.az[i]); v = f.vz[i] + dv; f.vz[i] = v; f.az[i] = a; d2 += dv * dv; v2 += v * v;
+        a = ndu[i]; f.u[i] = f.u[i] + hdt * (a - f.du[i]); f.du[i] = a;
+    }
+    if (ERR) {
+        __shared__ double smax[8], ssum[8];
+        d2 = warp_max(d2);
+        v2 = warp_sum(v2);
+        if (lane_id() == 0) { smax[threadIdx.x >> 5] = d2; ssum[threadIdx.x >> 5] = v2; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double m = smax[0], t = ssum[0];
+            for (int w = 1; w < 8; ++w) { m = fmax(m, smax[w]); t += ssum[w]; }
+            part_max[blockIdx.x] = m;
+            part_sum[blockIdx.x] = t;
+        }
+    }
+}
+
+// second stage of the corrector-check reduction: one block, fixed order (bitwise reproducible)
+__global__ void __launch_bounds__(256) k_corr_final(int nblocks, const double* __restrict__ part_max,
+                                                    const double* __restrict__ part_sum, DevScalars* sc) {
+    __shared__ double smax[256], ssum[256];
+    double m = 0.0, t = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 256) { m = fmax(m, part_max[b]); t += part_sum[b]; }
+    smax[threadIdx.x] = m; ssum[threadIdx.x] = t;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) {
+            smax[threadIdx.x] = fmax(smax[threadIdx.x], smax[threadIdx.x + w]);
+            ssum[threadIdx.x] += ssum[threadIdx.x + w];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { sc->corr_dvmax2 = smax[0]; sc->corr_v2sum = ssum[0]; }
 }
 
 // copy a^{n+1} into the a^n slots without a velocity correction (white step)
@@ -74,8 +112,8 @@ __global__ void __launch_bounds__(256) k_hmax(int64_t N, const double* __restric
 }
 __global__ void k_hmax_reset(DevScalars* sc) { sc->h_max = 0.0; }
 
-__global__ void k_set_dt(double* dtp, DevScalars* sc, double user_dt) {
-    const double dt = (user_dt > 0.0) ? user_dt : sc->dt;
+__global__ void k_set_dt(double* dtp, DevScalars* sc, double user_dt, double cfl_mult) {
+    const double dt = (user_dt > 0.0) ? user_dt : cfl_mult * sc->dt;       // G9: both terms of G8 are linear in the C's
     *dtp = dt;
     sc->t += dt;
 }
@@ -92,8 +130,16 @@ int launch_predict(sph_ctx* c) {
     return SPH_OK;
 }
 
-int launch_correct(sph_ctx* c) {
-    k_correct<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu, c->d_dtstep);
+int launch_correct(sph_ctx* c, bool with_check) {
+    const unsigned nb = div_up(c->N, 256);
+    if (with_check) {
+        k_correct<true><<<nb, 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu, c->d_dtstep, c->corr_part,
+                                                   c->corr_part + nb);
+        k_corr_final<<<1, 256, 0, c->stream>>>((int)nb, c->corr_part, c->corr_part + nb, c->d_sc);
+        c->launches++;
+    } else {
+        k_correct<false><<<nb, 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu, c->d_dtstep, nullptr, nullptr);
+    }
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -116,7 +162,7 @@ int launch_adopt_acc(sph_ctx* c) {
 }
 
 int launch_set_dt(sph_ctx* c, double user_dt) {
-    k_set_dt<<<1, 1, 0, c->stream>>>(c->d_dtstep, c->d_sc, user_dt);
+    k_set_dt<<<1, 1, 0, c->stream>>>(c->d_dtstep, c->d_sc, user_dt, c->cfl_mult);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -52,6 +52,7 @@ class Workload:
     point_mass: tuple | None = None  # (GM, softening, (cx, cy, cz))
     steps: int = 1
     cfl: tuple | None = None  # (C_cour, C_force) if not the defaults (Sedov blast)
+    eps_v: float | None = None  # leapfrog corrector check G7; None / 0 = off
 
     @property
     def n(self) -> int:
@@ -155,8 +156,8 @@ def sedov(n_side: int = 128, E0: float = 1.0, cfl: float = 0.1, gamma: float = 5
     sites along x (row and layer counts rounded to even numbers and the y, z spacings stretched by a few per cent,
     less as n_side grows, so that the lattice is periodic), equal masses, and the energy E0 = 1 injected at the centre as u_a = E0 W(r_a, 2 h0)
     with the M4 kernel and h0 = hfact (m/rho)^(1/3) (the relaxed h of the lattice to 3e-4); u = 0 elsewhere.
-    ``cfl`` sets both C_cour and C_force (0.1 for the physics run, 1e-3 for the paper's timing run). The leapfrog
-    corrector re-cycle (G6-G10) is not built, so this is for short timing / parity runs."""
+    ``cfl`` sets both C_cour and C_force (0.1 for the physics run, 1e-3 for the paper's timing run); set
+    ``eps_v`` on the result to switch on the leapfrog corrector re-cycle (G6-G10)."""
     L = 1.2
     nx = int(n_side)
     dx = L / nx

@@ -39,7 +39,8 @@ def test_default_params_match_header_citations(lib):
     assert (p.hfact, p.chi, p.lambda_, p.eps_h) == (1.2, 1.1, 1.2, 1e-6)
     assert (p.alpha_av, p.beta_av, p.beta_u, p.c_cour, p.c_force) == (1.0, 2.0, 1.0, 0.3, 0.25)
     assert p.gamma == pytest.approx(5.0 / 3.0) and p.max_h_iter == 50 and p.max_restarts == 50 and p.eos == 0
-    assert C.sizeof(binding.Params) == 10 * 8 + 4 * 4 + 5 * 8 + 3 * 8
+    assert (p.eps_v, p.lambda_stiff, p.max_recycle) == (0.0, 2.0, 10)      # corrector re-cycle off by default
+    assert C.sizeof(binding.Params) == 10 * 8 + 4 * 4 + 5 * 8 + 3 * 8 + 2 * 8 + 2 * 4
     assert C.sizeof(binding.Box) == 6 * 8 + 3 * 4 + 4   # padded to 8
 
 

@@ -506,3 +506,28 @@ def test_long_run_conservation_and_reproducibility():
     _, g, _ = run()
     for k in f:
         assert np.array_equal(f[k], g[k]), k
+
+
+def test_corrector_recycle_parity():
+    """Leapfrog corrector check with re-cycle and CFL multiplier (G6-G10; readings A15, A16) on the Sedov set-up at
+    C = 0.3, where the check fires in the first steps: re-cycle counts, multiplier, dt and fields follow the oracle."""
+    w = W.sedov(20, cfl=0.3)
+    w.eps_v = 1e-2
+    sim = _sim(w)
+    s = O.State(w, "grid")
+    seen = []
+    for _ in range(6):
+        dt_gpu = sim.step_leapfrog(want_dt=True)
+        dt_or = s.step()
+        st = sim.stats()
+        assert dt_gpu == pytest.approx(dt_or, rel=1e-9)
+        assert st["recycles"] == s.recycles and st["cfl_mult"] == pytest.approx(s.cfl_mult, rel=1e-14)
+        assert st["dt"] == pytest.approx(s.dt, rel=1e-9)
+        seen.append(s.recycles)
+    assert max(seen) > 0 and min(seen) == 0
+    g = _np(sim.get_fields())
+    assert np.max(np.abs(g["pos"] - s.pos)) < 1e-10
+    assert np.max(np.abs(g["vel"] - s.vel)) < 1e-8 * np.abs(s.vel).max()
+    assert np.max(np.abs(g["u"] - s.u)) < 1e-8 * np.abs(s.u).max()
+    assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
+    sim.close()

@@ -384,3 +384,42 @@ def test_sod_tube_against_exact_riemann():
     l1 = lambda a, b: np.mean(np.abs(a - b))
     assert l1(s.rho[sel], rho_e) < 0.04 and l1(s.vel[0][sel], v_e) < 0.06 and l1(P[sel], p_e) < 0.04
     assert np.abs(s.vel[1:]).max() < 0.01
+
+
+def test_corrector_recycle_pins():
+    """Leapfrog corrector check / re-cycle (G6-G7, reading A15) and CFL multiplier (G9-G10).
+    Pins that do not restate the code: (i) with the check switched off, or a threshold nothing can reach, the step
+    is bit-identical to the plain G1-G5 step; (ii) re-cycling is the fixed-point iteration of the implicit corrector
+    v = v* + dt/2 (a(v) - a^n): the change between k and k+1 forced re-cycles shrinks geometrically; (iii) the
+    multiplier halves after a step that re-cycled and relaxes as (1 + s m)/(1 + s) otherwise."""
+    import oracle as O
+    from paper_2503_09713_b200 import workloads as W
+    w = W.sedov(12, cfl=0.3)
+
+    def run(steps, **kw):
+        s = O.State(w, "grid", **kw)
+        out = []
+        for _ in range(steps):
+            s.step()
+            out.append((s.recycles, s.cfl_mult))
+        return s, out
+
+    plain, _ = run(2)
+    off, rec = run(2, eps_v=1e30)
+    assert np.array_equal(plain.vel, off.vel) and np.array_equal(plain.u, off.u) and np.array_equal(plain.pos, off.pos)
+    assert [r for r, _ in rec] == [0, 0] and rec[-1][1] == 1.0
+    # (ii) force exactly k re-cycles in the first step
+    vk = []
+    for k in range(5):
+        s, rec = run(1, eps_v=1e-300, max_recycle=k)
+        assert rec[0][0] == k
+        vk.append(s.vel.copy())
+    d = [np.abs(vk[k + 1] - vk[k]).max() for k in range(4)]
+    assert d[0] > 0 and all(d[k + 1] < 0.5 * d[k] for k in range(3))
+    # (iii) multiplier
+    s, rec = run(6, eps_v=1e-2, lambda_stiff=2.0)
+    m = 1.0
+    for r, mult in rec:
+        m = 0.5 * m if r > 0 else (1.0 + 2.0 * m) / 3.0
+        assert mult == pytest.approx(m, rel=1e-15)
+    assert any(r > 0 for r, _ in rec) and any(r == 0 for r, _ in rec)
