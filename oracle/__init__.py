@@ -38,7 +38,7 @@ class Params(C.Structure):
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("newton_literal", C.c_int32),
                 ("cs0", C.c_double), ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
                 ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
-                ("max_recycle", C.c_int32), ("pad_", C.c_int32)]
+                ("max_recycle", C.c_int32), ("kernel", C.c_int32)]
 
 
 def make_box(lo, hi, periodic) -> Box:
@@ -47,12 +47,12 @@ def make_box(lo, hi, periodic) -> Box:
 
 def make_params(gamma=5.0 / 3.0, hfact=1.2, chi=1.1, lam=1.2, eps_h=1e-6, alpha_av=1.0, beta_av=2.0, beta_u=1.0,
                 c_cour=0.3, c_force=0.25, max_h_iter=50, max_restarts=50, eos_isothermal=None, point_mass=None,
-                newton_literal=0, eps_v=0.0, lambda_stiff=2.0, max_recycle=10) -> Params:
+                newton_literal=0, eps_v=0.0, lambda_stiff=2.0, max_recycle=10, kernel=0) -> Params:
     p = Params()
     p.hfact, p.gamma, p.chi, p.lam, p.eps_h = hfact, gamma, chi, lam, eps_h
     p.alpha_av, p.beta_av, p.beta_u, p.c_cour, p.c_force = alpha_av, beta_av, beta_u, c_cour, c_force
     p.max_h_iter, p.max_restarts, p.newton_literal = max_h_iter, max_restarts, newton_literal
-    p.eps_v, p.lambda_stiff, p.max_recycle = eps_v, lambda_stiff, max_recycle
+    p.eps_v, p.lambda_stiff, p.max_recycle, p.kernel = eps_v, lambda_stiff, max_recycle, kernel
     p.eos = 0
     if eos_isothermal is not None:
         p.eos = 1
@@ -70,6 +70,8 @@ def workload_box_params(w, **kw):
         kw = dict(dict(c_cour=cfl[0], c_force=cfl[1]), **kw)
     if getattr(w, "eps_v", None):
         kw = dict(dict(eps_v=w.eps_v), **kw)
+    if getattr(w, "kernel", 0):
+        kw = dict(dict(kernel=w.kernel), **kw)
     return (make_box(w.box_lo, w.box_hi, w.periodic),
             make_params(gamma=w.gamma, hfact=w.hfact, eos_isothermal=w.eos_isothermal, point_mass=w.point_mass, **kw))
 
@@ -154,11 +156,17 @@ def aabb(t, pos_sorted, h_sorted):
     return box6, hmax
 
 
-def neighbours(pos, h, box: Box, chi=1.1, mode="brute"):
+def set_kernel(k: int = 0):
+    """Select the SPH kernel of every later oracle call: 0 = M4, 1 = M5, 2 = M6 (file-level selector in the C++)."""
+    lib().orc_set_kernel(C.c_int32(int(k)))
+
+
+def neighbours(pos, h, box: Box, chi=1.1, mode="brute", kernel=0):
     """CSR neighbour sets N(a) (self included, each list ascending): (offs u64[N+1], idx u32[total])."""
     pos = _f64(pos)
     h = _f64(h)
     n = pos.shape[1]
+    set_kernel(kernel)
     fn = lib().orc_neighbours_brute if mode == "brute" else lib().orc_neighbours_grid
     offs = np.empty(n + 1, dtype=np.uint64)
     total = fn(C.c_int64(n), _p(pos, np.float64), _p(h, np.float64), C.byref(box), C.c_double(chi),
@@ -175,6 +183,7 @@ def density(pos, m, hn, offs, idx, box: Box, p: Params):
     n = pos.shape[1]
     out = dict(h=np.empty(n), rho=np.empty(n), omega=np.empty(n), iters=np.empty(n, np.int32),
                exceeded=np.empty(n, np.uint8))
+    set_kernel(p.kernel)
     ne = lib().orc_density(C.c_int64(n), _p(pos, np.float64), _p(m, np.float64), _p(hn, np.float64),
                            _p(offs, np.uint64), _p(idx, np.uint32), C.byref(box), C.byref(p), _p(out["h"], np.float64),
                            _p(out["rho"], np.float64), _p(out["omega"], np.float64), _p(out["iters"], np.int32),
@@ -183,10 +192,11 @@ def density(pos, m, hn, offs, idx, box: Box, p: Params):
     return out
 
 
-def h_bisect(pos, m, box: Box, hfact, h_lo, h_hi):
+def h_bisect(pos, m, box: Box, hfact, h_lo, h_hi, kernel=0):
     pos, m, h_lo, h_hi = _f64(pos), _f64(m), _f64(h_lo), _f64(h_hi)
     n = pos.shape[1]
     out = np.empty(n)
+    set_kernel(kernel)
     lib().orc_h_bisect(C.c_int64(n), _p(pos, np.float64), _p(m, np.float64), C.byref(box), C.c_double(hfact),
                        _p(h_lo, np.float64), _p(h_hi, np.float64), _p(out, np.float64))
     return out
@@ -197,6 +207,7 @@ def forces(pos, vel, m, h, rho, omega, u, offs, idx, box: Box, p: Params):
     n = pos.shape[1]
     acc = np.empty((3, n))
     dudt = np.empty(n)
+    set_kernel(p.kernel)
     dt = lib().orc_forces(C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(m, np.float64),
                           _p(h, np.float64), _p(rho, np.float64), _p(omega, np.float64), _p(u, np.float64),
                           _p(offs, np.uint64), _p(idx, np.uint32), C.byref(box), C.byref(p), _p(acc, np.float64),
@@ -215,6 +226,7 @@ def evaluate(pos, vel, m, u, h, box: Box, p: Params, mode="grid"):
     out = dict(h=h, rho=np.empty(n), omega=np.empty(n), acc=np.empty((3, n)), dudt=np.empty(n))
     dt = C.c_double()
     nn = C.c_int64()
+    set_kernel(p.kernel)
     rc = lib().orc_evaluate(C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(m, np.float64),
                             _p(u, np.float64), _p(h, np.float64), C.byref(box), C.byref(p),
                             C.c_int32(0 if mode == "brute" else 1), _p(out["rho"], np.float64),
@@ -247,6 +259,7 @@ class State:
         dtn = C.c_double()
         mult = C.c_double(getattr(self, "cfl_mult", 1.0))
         nrec = C.c_int32()
+        set_kernel(self.p.kernel)
         rc = lib().orc_step2(C.c_int64(n), _p(self.pos, np.float64), _p(self.vel, np.float64), _p(self.m, np.float64),
                              _p(self.u, np.float64), _p(self.h, np.float64), _p(self.acc, np.float64),
                              _p(self.dudt, np.float64), C.byref(self.box), C.byref(self.p),

@@ -53,24 +53,34 @@ struct orc_params {
     double eps_v;        // leapfrog corrector check G7: 1e-2 in the paper; 0 disables (reading A15)
     double lambda_stiff; // stiffness of the CFL multiplier G10; value not given, reading A16
     int32_t max_recycle; // cap on corrector re-cycles per step
-    int32_t pad_;
+    int32_t kernel;      // 0 = M4, 1 = M5, 2 = M6 (informational here: the selector is orc_set_kernel)
 };
 
 }  // extern "C"
 
 namespace {
 
-constexpr double kRkern = 2.0;                       // M4 support radius in units of h
-constexpr double kCnorm = 0.31830988618379067154;    // 1/pi, 3-D M4 normalisation (reading O6)
+// ---- O6: Schoenberg (1946) B-spline kernels M4 (cubic), M5 (quartic), M6 (quintic); the paper names them
+// (M6 with h_fact = 1.0 in its physics tests) but prints neither f nor C_norm: textbook
+// forms, q = r/h, 3-D normalisations 1/pi, 1/(20 pi), 1/(120 pi), support radii 2, 2.5, 3.
+// The kernel in use is a file-level selector set through orc_set_kernel (test infrastructure, single-threaded);
+// 0 = M4 (default), 1 = M5, 2 = M6.
+int g_kernel = 0;
+#define kRkern (g_kernel == 0 ? 2.0 : g_kernel == 1 ? 2.5 : 3.0)
+#define kCnorm (g_kernel == 0 ? 0.31830988618379067154 : g_kernel == 1 ? 0.31830988618379067154 / 20.0 : 0.31830988618379067154 / 120.0)
 
-// ---- O6: M4 cubic B-spline (Schoenberg 1946; the paper names M4, but prints neither f nor
-// C_norm: textbook form). q = r/h.
-inline double f_m4(double q) {
+inline double pw(double x, int n) { double r = 1.0; for (int i = 0; i < n; ++i) r *= x; return x > 0.0 ? r : 0.0; }
+
+inline double f_m4(double q) {          // f(q) of the selected kernel (name kept from the M4-only version)
+    if (g_kernel == 1) return pw(2.5 - q, 4) - 5.0 * pw(1.5 - q, 4) + 10.0 * pw(0.5 - q, 4);
+    if (g_kernel == 2) return pw(3.0 - q, 5) - 6.0 * pw(2.0 - q, 5) + 15.0 * pw(1.0 - q, 5);
     if (q < 1.0) return 1.0 - 1.5 * q * q + 0.75 * q * q * q;
     if (q < 2.0) { double t = 2.0 - q; return 0.25 * t * t * t; }
     return 0.0;
 }
-inline double df_m4(double q) {
+inline double df_m4(double q) {         // f'(q)
+    if (g_kernel == 1) return -4.0 * (pw(2.5 - q, 3) - 5.0 * pw(1.5 - q, 3) + 10.0 * pw(0.5 - q, 3));
+    if (g_kernel == 2) return -5.0 * (pw(3.0 - q, 4) - 6.0 * pw(2.0 - q, 4) + 15.0 * pw(1.0 - q, 4));
     if (q < 1.0) return -3.0 * q + 2.25 * q * q;
     if (q < 2.0) { double t = 2.0 - q; return -0.75 * t * t; }
     return 0.0;
@@ -184,6 +194,7 @@ inline void eos(const orc_params& p, double rho, double u, double x, double y, d
 extern "C" {
 
 // ---- exported scalar kernel functions (pins: quadrature, continuity, W(0)) ----
+void orc_set_kernel(int32_t k) { g_kernel = (k == 1 || k == 2) ? k : 0; }
 double orc_f(double q) { return f_m4(q); }
 double orc_df(double q) { return df_m4(q); }
 double orc_W(double r, double h) { return W(r, h); }

@@ -40,7 +40,7 @@ class Params(C.Structure):
     _fields_ = [("hfact", C.c_double), ("gamma", C.c_double), ("chi", C.c_double), ("lambda_", C.c_double),
                 ("eps_h", C.c_double), ("alpha_av", C.c_double), ("beta_av", C.c_double), ("beta_u", C.c_double),
                 ("c_cour", C.c_double), ("c_force", C.c_double), ("max_h_iter", C.c_int32),
-                ("max_restarts", C.c_int32), ("eos", C.c_int32), ("reserved", C.c_int32), ("cs0", C.c_double),
+                ("max_restarts", C.c_int32), ("eos", C.c_int32), ("kernel", C.c_int32), ("cs0", C.c_double),
                 ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
                 ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
                 ("max_recycle", C.c_int32), ("reserved2", C.c_int32)]
@@ -125,6 +125,8 @@ def params_for(w, **kw) -> Params:
         extra.update(c_cour=w.cfl[0], c_force=w.cfl[1])
     if getattr(w, "eps_v", None):
         extra.update(eps_v=w.eps_v)
+    if getattr(w, "kernel", 0):
+        extra.update(kernel=w.kernel)
     extra.update(kw)
     return default_params(**extra)
 

@@ -134,9 +134,9 @@ static int cache_build(sph_ctx* c) {
         SPH_TRY(read_scalars(c));
         const DevScalars& s = *c->h_sc;
         for (int k = 0; k < 3; ++k)
-            if (c->box.periodic[k] && !(2.0 * kRkern * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
+            if (c->box.periodic[k] && !(2.0 * kern_radius(c->p.kernel) * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
                 return fail(c, SPH_ERR_PERIODIC_TOO_SMALL, "periodic axis %d: 2 R_kern chi h_max = %g >= L = %g", k,
-                            2.0 * kRkern * c->p.chi * s.h_max, c->box.hi[k] - c->box.lo[k]);
+                            2.0 * kern_radius(c->p.kernel) * c->p.chi * s.h_max, c->box.hi[k] - c->box.lo[k]);
         if (s.n_cand_overflow)
             return fail(c, SPH_ERR_CAP, "%u leaf groups have more than 65535 candidates (16-bit local index)",
                         s.n_cand_overflow);
@@ -183,7 +183,7 @@ void sph_default_params(sph_params* p) {
     memset(p, 0, sizeof(*p));
     p->hfact = 1.2; p->gamma = 5.0 / 3.0; p->chi = 1.1; p->lambda = 1.2; p->eps_h = 1e-6;
     p->alpha_av = 1.0; p->beta_av = 2.0; p->beta_u = 1.0; p->c_cour = 0.3; p->c_force = 0.25;
-    p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0;
+    p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0; p->kernel = 0;
     p->cs0 = 1.0; p->r0 = 1.0; p->q = 0.0; p->GM = 0.0; p->soft = 0.0;
     p->eps_v = 0.0; p->lambda_stiff = 2.0; p->max_recycle = 10;
 }
@@ -221,6 +221,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     c->N = N;
     c->box = *box;
     if (params) c->p = *params; else sph_default_params(&c->p);
+    if (c->p.kernel < 0 || c->p.kernel > 2) return fail(c, SPH_ERR_ARG, "kernel must be 0 (M4), 1 (M5) or 2 (M6)");
     if (!(c->p.hfact > 0) || !(c->p.chi >= 1.0) || !(c->p.lambda > 1.0) || !(c->p.eps_h > 0) || c->p.max_h_iter < 1)
         return fail(c, SPH_ERR_ARG, "bad parameters");
     c->stream = (cudaStream_t)cuda_stream;

@@ -16,8 +16,12 @@
 namespace sph {
 
 constexpr int kGroup = 32;          // leaf-group size bound: one warp lane per particle of a group
-constexpr double kRkern = 2.0;      // M4 support radius / h
-constexpr double kCnorm = 0.31830988618379067154;   // 1/pi
+// B-spline kernels (reading O6): 0 = M4 (cubic), 1 = M5 (quartic), 2 = M6 (quintic);
+// support radius in units of h and 3-D normalisation 1/pi, 1/(20 pi), 1/(120 pi)
+__host__ __device__ constexpr double kern_radius(int k) { return k == 0 ? 2.0 : (k == 1 ? 2.5 : 3.0); }
+__host__ __device__ constexpr double kern_cnorm(int k) {
+    return k == 0 ? 0.31830988618379067154 : (k == 1 ? 0.31830988618379067154 / 20.0 : 0.31830988618379067154 / 120.0);
+}
 
 // Sorted-order particle fields (SoA). Two sets are kept; the permute writes the other one.
 struct Fields {
@@ -211,6 +215,27 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // M4 cubic B-spline f(q) and f'(q) (reading O6); branch-light form.
+__device__ __forceinline__ void m4(double q, double& f, double& df);
+// f(q) and f'(q) of kernel K. M5 and M6 in clamped-power form: f = sum_i c_i (a_i - q)_+^p
+template <int K>
+__device__ __forceinline__ void kern_f_df(double q, double& f, double& df) {
+    if (K == 0) {
+        m4(q, f, df);
+    } else if (K == 1) {
+        const double a = 2.5 - q, b = 1.5 - q, c = 0.5 - q;
+        const double t1 = a > 0.0 ? a : 0.0, t2 = b > 0.0 ? b : 0.0, t3 = c > 0.0 ? c : 0.0;
+        const double c1 = t1 * t1 * t1, c2 = t2 * t2 * t2, c3 = t3 * t3 * t3;
+        f = fma(10.0 * c3, t3, fma(-5.0 * c2, t2, c1 * t1));
+        df = -4.0 * fma(10.0, c3, fma(-5.0, c2, c1));
+    } else {
+        const double a = 3.0 - q, b = 2.0 - q, c = 1.0 - q;
+        const double t1 = a > 0.0 ? a : 0.0, t2 = b > 0.0 ? b : 0.0, t3 = c > 0.0 ? c : 0.0;
+        const double s1 = t1 * t1, s2 = t2 * t2, s3 = t3 * t3;
+        const double q1 = s1 * s1, q2 = s2 * s2, q3 = s3 * s3;
+        f = fma(15.0 * q3, t3, fma(-6.0 * q2, t2, q1 * t1));
+        df = -5.0 * fma(15.0, q3, fma(-6.0, q2, q1));
+    }
+}
 __device__ __forceinline__ void m4(double q, double& f, double& df) {
     double t2 = 2.0 - q;
     double fo = 0.25 * t2 * t2 * t2;          // outer branch 1 <= q < 2

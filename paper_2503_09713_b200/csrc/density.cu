@@ -54,7 +54,7 @@ struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 // and the per-neighbour mass registers disappear.
 // GLOB: the candidate array is too large to stage; sx, sy, sz, sm are the global field arrays and a candidate index
 // is translated through the group's candidate array cs first.
-template <bool WRAP, bool UNIM, bool GLOB>
+template <bool WRAP, bool UNIM, bool GLOB, int K>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
                                             const uint32_t* __restrict__ cs,
                                             const uint16_t* __restrict__ li, const uint32_t (&idx)[(kRegChunks + 1) / 2],
@@ -82,7 +82,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
 #pragma unroll
         for (int c = 0; c < kRegChunks; ++c) {
             double qq = r[c] * hinv, f, df;
-            m4(qq, f, df);
+            kern_f_df<K>(qq, f, df);
             if (UNIM) {
                 rs += f;
                 ss += fma(qq, df, 3.0 * f);
@@ -96,13 +96,13 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
             if (GLOB) b = cs[b];
             double qq = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, df;
             const double mm = UNIM ? 1.0 : sm[b];
-            m4(qq, f, df);
+            kern_f_df<K>(qq, f, df);
             rs = fma(mm, f, rs);
             ss = fma(mm, fma(qq, df, 3.0 * f), ss);
         }
         rs = octet_sum(rs);
         ss = octet_sum(ss);
-        const double c3 = (UNIM ? m0 : 1.0) * kCnorm * hinv * hinv * hinv;
+        const double c3 = (UNIM ? m0 : 1.0) * kern_cnorm(K) * hinv * hinv * hinv;
         rho_sum = c3 * rs;            // Eq. 1-2
         S = -c3 * hinv * ss;          // sum_b m_b dW/dh
     };
@@ -144,8 +144,8 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     out.it = it;
 }
 
-template <bool UNIM, bool GLOB>
-__global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
+template <bool UNIM, bool GLOB, int K>
+__global__ void __launch_bounds__(kDensWarps * 32, (UNIM && K == 0) ? 3 : 2) k_density(
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
     const GroupRec* __restrict__ ginfo, const uint32_t* __restrict__ cslot, const uint32_t* __restrict__ cnt,
@@ -197,8 +197,8 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
     __syncthreads();
 
     DensOut o;
-    if (gwrap) octet_solve<true, UNIM, GLOB>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
-    else octet_solve<false, UNIM, GLOB>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    if (gwrap) octet_solve<true, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    else octet_solve<false, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
 
     if (pv && sl == 0u) {
         hout[a] = o.h;
@@ -219,22 +219,29 @@ __global__ void __launch_bounds__(kDensWarps * 32, UNIM ? 3 : 2) k_density(
 
 __global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; }
 
-template <bool UNIM, bool GLOB>
-static void density_launch(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
-                           uint32_t hi) {
-    k_density<UNIM, GLOB><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
+template <bool UNIM, bool GLOB, int K>
+static void density_launch_k(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
+                             uint32_t hi) {
+    static bool attr_set = false;
+    if (!attr_set && !GLOB) {
+        cudaFuncSetAttribute(k_density<UNIM, GLOB, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        attr_set = true;
+    }
+    k_density<UNIM, GLOB, K><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
         c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db, dp,
         ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
     c->launches++;
 }
 
+template <bool UNIM, bool GLOB>
+static void density_launch(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
+                           uint32_t hi) {
+    if (c->p.kernel == 0) density_launch_k<UNIM, GLOB, 0>(c, smem, db, dp, ncap, lo, hi);
+    else if (c->p.kernel == 1) density_launch_k<UNIM, GLOB, 1>(c, smem, db, dp, ncap, lo, hi);
+    else density_launch_k<UNIM, GLOB, 2>(c, smem, db, dp, ncap, lo, hi);
+}
+
 int launch_density(sph_ctx* c) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        SPH_CUDA(c, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_set = true;
-    }
     DensBox db;
     for (int k = 0; k < 3; ++k) {
         db.L[k] = c->box.hi[k] - c->box.lo[k];

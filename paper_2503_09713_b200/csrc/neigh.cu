@@ -536,7 +536,7 @@ int launch_traverse(sph_ctx* c) {
         Lmax = fmax(Lmax, tb.L[k]);
     }
     tb.gg_pad = 1e-14 * Lmax;
-    const double rk_chi = kRkern * c->p.chi;
+    const double rk_chi = kern_radius(c->p.kernel) * c->p.chi;
     TravOut out;
     out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
     out.cslot = c->cslot; out.cslot_cap = c->cslot_cap; out.scratch = c->trav_scratch; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;

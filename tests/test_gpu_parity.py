@@ -76,7 +76,7 @@ def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None):
     if ev["restarts"] == 0:
         assert np.array_equal(g["hmax"], hmax), "node hmax differs"
         # a4: neighbour sets (sorted-slot indices), compared as sets per particle
-        oo, oi = O.neighbours(ps, hn[gperm], box, p.chi, "grid")
+        oo, oi = O.neighbours(ps, hn[gperm], box, p.chi, "grid", kernel=p.kernel)
         go, gi = sim.get_neighbours()
         assert _near_cutoff_pairs(ps, hn[gperm], box, p.chi, oo, oi) == 0   # nothing to exclude on these inputs
         assert np.array_equal(go, oo), "neighbour counts differ"
@@ -531,3 +531,23 @@ def test_corrector_recycle_parity():
     assert np.max(np.abs(g["u"] - s.u)) < 1e-8 * np.abs(s.u).max()
     assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
     sim.close()
+
+
+@pytest.mark.parametrize("kernel,hfact", [(1, 1.2), (2, 1.0)], ids=["M5", "M6_hfact1"])
+def test_other_kernels_stage_and_step_parity(kernel, hfact):
+    """M5 and M6 B-spline kernels (M6 with h_fact = 1.0 is the paper's physics-test setting,
+    PAPER.md:208): support radii 2.5 and 3 enter the traversal, the kernels the density and force loops."""
+    w = W.cube(14, jitter=0.08, vel_amp=0.03, seed=9)
+    w.kernel, w.hfact = kernel, hfact
+    w.h0 = np.full(w.n, hfact / 14)
+    sim = _sim(w)
+    ev, f = _stage_parity(w, sim)
+    assert ev["n_neigh"] / w.n > (100 if kernel == 1 else 130)
+    s = O.State(w, "grid")
+    for _ in range(2):
+        assert sim.step_leapfrog(want_dt=True) == pytest.approx(s.step(), rel=1e-9)
+    g = _np(sim.get_fields())
+    assert np.max(np.abs(g["pos"] - s.pos)) < 1e-12 and np.max(np.abs(g["h"] / s.h - 1)) < 1e-9
+    assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
+    sim.close()
+    O.set_kernel(0)

@@ -84,22 +84,48 @@ def test_group_criterion_is_conservative():
 
 # ---------------------------------------------------------------- kernel (O6)
 
-def test_m4_kernel_closed_forms():
+@pytest.mark.parametrize("kernel,radius,f0,cnorm", [(0, 2.0, 1.0, 1.0 / math.pi), (1, 2.5, 14.375, 1.0 / (20.0 * math.pi)),
+                                                     (2, 3.0, 66.0, 1.0 / (120.0 * math.pi))], ids=["M4", "M5", "M6"])
+def test_kernel_closed_forms(kernel, radius, f0, cnorm):
+    """B-spline kernels M4, M5, M6: unit volume integral (pins the 3-D normalisations 1/pi, 1/(20 pi),
+    1/(120 pi)), closed-form central values (1, 115/8, 66), compact support, continuity of f and f' at the knots,
+    F and dW/dh against finite differences of W."""
     L = O.lib()
-    r = np.linspace(0.0, 2.0, 200001)
-    f = np.array([L.orc_f(q) for q in r])
-    integral = np.trapezoid(4.0 * math.pi * r * r * f / math.pi, r)      # int W dV with h = 1
-    assert abs(integral - 1.0) < 1e-9
-    assert L.orc_W(0.0, 0.7) == pytest.approx(1.0 / (math.pi * 0.7 ** 3), rel=1e-15)
-    for q in (1.0, 2.0):
-        assert L.orc_f(q - 1e-12) == pytest.approx(L.orc_f(q + 1e-12), abs=1e-11)
-        assert L.orc_df(q - 1e-12) == pytest.approx(L.orc_df(q + 1e-12), abs=1e-11)
-    assert L.orc_f(2.5) == 0.0 and L.orc_df(2.5) == 0.0
-    for rr, h in ((0.3, 0.5), (0.7, 0.5), (0.2, 1.3)):
-        eps = 1e-6
-        assert L.orc_F(rr, h) == pytest.approx((L.orc_W(rr + eps, h) - L.orc_W(rr - eps, h)) / (2 * eps), rel=1e-8)
-        assert L.orc_dWdh(rr, h) == pytest.approx((L.orc_W(rr, h + eps) - L.orc_W(rr, h - eps)) / (2 * eps), rel=1e-8)
-    assert L.orc_df(0.5) < 0 and L.orc_df(1.5) < 0
+    O.set_kernel(kernel)
+    try:
+        r = np.linspace(0.0, radius, 300001)
+        f = np.array([L.orc_f(q) for q in r])
+        assert abs(np.trapezoid(4.0 * math.pi * r * r * f * cnorm, r) - 1.0) < 1e-9           # int W dV with h = 1
+        assert L.orc_W(0.0, 0.7) == pytest.approx(f0 * cnorm / 0.7 ** 3, rel=1e-15)
+        for q in np.arange(radius, 0.0, -1.0):
+            assert L.orc_f(q - 1e-12) == pytest.approx(L.orc_f(q + 1e-12), abs=1e-9)
+            assert L.orc_df(q - 1e-12) == pytest.approx(L.orc_df(q + 1e-12), abs=1e-9)
+        assert L.orc_f(radius + 0.5) == 0.0 and L.orc_df(radius + 0.5) == 0.0 and L.orc_f(radius - 1e-3) > 0.0
+        for rr, h in ((0.3, 0.5), (0.7, 0.5), (0.2, 1.3)):
+            eps = 1e-6
+            assert L.orc_F(rr, h) == pytest.approx((L.orc_W(rr + eps, h) - L.orc_W(rr - eps, h)) / (2 * eps), rel=1e-7)
+            assert L.orc_dWdh(rr, h) == pytest.approx((L.orc_W(rr, h + eps) - L.orc_W(rr, h - eps)) / (2 * eps), rel=1e-7)
+        assert all(L.orc_df(q) < 0 for q in (0.25, 0.75, 1.5, radius - 0.2)) and L.orc_df(0.0) == 0.0
+    finally:
+        O.set_kernel(0)
+
+
+def test_m6_lattice_and_conservation():
+    """M6 with h_fact = 1.0 (the paper's physics-test setting: ~113 neighbours): uniform density on a
+    lattice, h from the unique-root bisection, momentum and energy identities."""
+    w = W.cube(10, jitter=0.03, vel_amp=0.05, seed=4)
+    w.hfact, w.kernel = 1.0, 2
+    w.h0 = np.full(w.n, 1.0 / 10)
+    box, p = O.workload_box_params(w)
+    ev = O.evaluate(w.pos, w.vel, w.mass, w.u, w.h0, box, p, "brute")
+    assert 105 < ev["n_neigh"] / w.n < 160 and abs(ev["rho"].mean() - 1.0) < 2e-3
+    hb = O.h_bisect(w.pos, w.mass, box, p.hfact, 0.5 * ev["h"], 2.0 * ev["h"], kernel=2)
+    assert np.max(np.abs(hb / ev["h"] - 1)) < 1e-6
+    ma = (w.mass * ev["acc"]).sum(axis=1)
+    assert np.all(np.abs(ma) < 1e-13 * np.abs(w.mass * ev["acc"]).sum(axis=1).max())
+    de = (w.mass * ((w.vel * ev["acc"]).sum(axis=0) + ev["dudt"])).sum()
+    assert abs(de) < 1e-12 * (w.mass * np.abs(ev["dudt"])).sum()
+    O.set_kernel(0)
 
 
 # ---------------------------------------------------------------- density / h (O7)
