@@ -249,6 +249,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
     SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
     SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
+    SPH_TRY(dalloc(c, &c->trav_hit_scratch, trav_hit_scratch_entries()));
     SPH_TRY(dalloc(c, &c->corr_part, 2 * (size_t)div_up(N, 256) + 2));
     // cache pools start empty: the first traversal only counts, then they are sized from its totals
     c->scan_tiles = scan_scratch_tiles(N);

@@ -117,6 +117,7 @@ struct sph_ctx {
     uint32_t* cslot = nullptr;          // candidate pool
     uint64_t cslot_cap = 0;
     uint32_t* trav_scratch = nullptr;   // per-warp candidate rows of the traversal grid
+    uint16_t* trav_hit_scratch = nullptr;   // per-warp spill rows of the hit buffers
     sph::GroupRec* ginfo = nullptr;     // one per group
     uint64_t ginfo_cap = 0;
     uint32_t nc_max = 0;
@@ -178,6 +179,7 @@ int launch_tree(sph_ctx* c);                                   // tree.cu   karr
 int launch_aabb(sph_ctx* c);                                   // tree.cu
 int launch_traverse(sph_ctx* c);                               // neigh.cu  single pass: walk, test, write cache
 int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out);
+size_t trav_hit_scratch_entries();                              // neigh.cu  u16 entries of the traversal's hit spill rows
 size_t trav_scratch_entries();                                  // neigh.cu  u32 entries of the traversal's scratch rows        // neigh.cu  group-local lists -> global CSR (getter)
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu

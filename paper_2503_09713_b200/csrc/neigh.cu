@@ -22,8 +22,9 @@
 //     candidate array. Hits are buffered in shared memory, candidate slots in a per-warp global scratch row, and
 //     both are written out coalesced once the group is complete; space comes from two bump allocators (count ->
 //     allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed). A group whose
-//     buffers overflow (a list longer than kHitCap, more than kScrCap candidates) allocates from its exact
-//     counts and walks a second time writing directly.
+//     lists outgrow the shared-memory rows spills them to a per-warp scratch in global memory; beyond that (lists
+//     longer than kSpillCap + kHitCap, more than kScrCap candidates) it allocates from its exact counts and walks a
+//     second time writing directly.
 #include <stdlib.h>
 
 #include "common.cuh"
@@ -39,6 +40,7 @@ constexpr int kHitSlack = 32;            // room for one more bucket beyond kHit
 constexpr int kHitStride = kHitCap + kHitSlack + 2;   // in u16: 73 words per lane row (odd: rows start in distinct banks)
 constexpr int kShare = 4;               // consecutive groups that share one tree walk
 constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
+constexpr int kSpillCap = 512;            // hits per lane that can spill from the shared-memory row to the warp's global scratch
 constexpr int kScrCap = 2048;            // candidate slots buffered per group (global scratch row of the warp)
 constexpr uint32_t kLeafBit = 0x80000000u;
 constexpr uint32_t kWrapBit = 0x80000000u;
@@ -66,6 +68,7 @@ struct TravOut {
     uint32_t* cslot;
     uint64_t cslot_cap;
     uint32_t* scratch;       // kScrCap entries per warp of the grid
+    uint16_t* hit_scratch;   // 32 x kSpillCap entries per warp of the grid: spilled parts of the hit rows
     GroupRec* ginfo;
     uint64_t ginfo_cap;
 };
@@ -99,7 +102,10 @@ struct GroupCtx {
     double gxl, gxh, gyl, gyh, gzl, gzh, ghm;
     double rc2g;          // (R_kern chi hmax_group)^2, for the per-candidate prefilter
     uint32_t nhit;        // per lane: hits so far (exact)
-    uint32_t wpos;        // per lane, buffered mode: store position in the lane's row (clamped to kHitCap per bucket)
+    uint32_t wpos;        // per lane, buffered mode: store position in the lane's row
+    uint32_t nspill;      // per lane, buffered mode: hits of this group already spilled to the warp's global scratch
+    bool hard_overflow;   // warp-uniform: a row could not spill any more (the group is walked a second time)
+    uint16_t* hspill;     // this lane's row of the warp's hit scratch
     uint32_t ncs;         // warp-uniform: candidates (prefilter survivors) so far
     uint16_t* lptr;       // DIRECT: this lane's list in global memory
     uint32_t* cptr;       // candidate slots: the warp's scratch row, or (DIRECT) the group's array in global memory
@@ -205,7 +211,19 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             const uint32_t got = (wp - w0) >> 1;
             G.nhit += got;
             G.wpos += got;
-            if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;   // overflowed row: keep counting, stop growing
+            // A row has room for one more bucket only up to kHitCap: when some lane is beyond it, every lane moves
+            // its row to its part of the warp's global scratch (the list order is kept: spilled part, then the row);
+            // when that is full too the group is counted on and walked a second time writing directly.
+            if (__any_sync(0xffffffffu, G.wpos > (uint32_t)kHitCap)) {
+                if (!G.hard_overflow && __all_sync(0xffffffffu, G.nspill + G.wpos <= (uint32_t)kSpillCap)) {
+                    for (uint32_t k = 0; k < G.wpos; ++k) G.hspill[G.nspill + k] = s.hits[row + k];
+                    G.nspill += G.wpos;
+                    G.wpos = 0u;
+                } else {
+                    G.hard_overflow = true;
+                    if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;
+                }
+            }
         }
         G.ncs += nk;
     }
@@ -294,7 +312,7 @@ __device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, uns
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.ncs = 0u; G.anywrap = false;
+    G.nhit = 0u; G.wpos = 0u; G.nspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
     int nb = 0;
     __syncwarp();
     for (int base = 0; base < nu; base += 32) {
@@ -323,7 +341,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.ncs = 0u; G.anywrap = false;
+    G.nhit = 0u; G.wpos = 0u; G.nspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
     int sp = 1, nb = 0;
     __syncwarp();
     if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
@@ -382,6 +400,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
     const unsigned lt = lanemask_lt();
     const uint32_t n_groups = sc->n_groups;
     unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u;
+    uint16_t* const hit_row = out.hit_scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * (32 * kSpillCap);
     uint32_t* const scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
 
     for (;;) {
@@ -437,6 +456,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         }
         if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
+        G.hspill = hit_row + (size_t)lane * kSpillCap;
 
         if (nu >= 0) refine<false>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
         else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
@@ -451,7 +471,6 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             if (lane >= (unsigned)o) incl += t;
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-        const uint32_t maxhit = warp_max_u32(nhit);
         unsigned long long lbase = 0, bbase = 0;
         if (lane == 0) {
             lbase = atomicAdd(&sc->list_cursor, (unsigned long long)((total + 7u) & ~7u));
@@ -474,15 +493,24 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                 r.nc = nc | (G.anywrap ? 0x80000000u : 0u); r.pad = 0u;
                 out.ginfo[g] = r;
             }
-            const bool overflow = (maxhit > (uint32_t)kHitCap) || (nc > (uint32_t)kScrCap);
+            const bool overflow = G.hard_overflow || (nc > (uint32_t)kScrCap);
             if (!overflow) {
                 __syncwarp();
                 for (uint32_t j = lane; j < nc; j += 32) out.cslot[bbase + j] = scr_row[j];
                 // lists: the warp copies one particle's buffered list at a time (coalesced 16-bit stores)
+                const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
                 for (uint32_t p = 0; p < nq; ++p) {
                     const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
-                    const uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - np);
-                    for (uint32_t k = lane; k < np; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
+                    uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - np);
+                    uint32_t nrow = np;
+                    if (spilled) {
+                        const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p);
+                        const uint16_t* src = hit_row + (size_t)p * kSpillCap;
+                        for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
+                        sp0 += ns;
+                        nrow = np - ns;
+                    }
+                    for (uint32_t k = lane; k < nrow; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
                 }
             } else {
                 // fallback: second walk writing directly at the now-known positions
@@ -519,6 +547,7 @@ __global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc) {
 
 constexpr int kTravBlocks = 148 * 2;     // persistent grid: two CTAs per SM (shared-memory bound)
 size_t trav_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * kScrCap; }
+size_t trav_hit_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * 32 * kSpillCap; }
 
 int launch_traverse(sph_ctx* c) {
     static bool attr_set = false;
@@ -539,7 +568,7 @@ int launch_traverse(sph_ctx* c) {
     const double rk_chi = kern_radius(c->p.kernel) * c->p.chi;
     TravOut out;
     out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
-    out.cslot = c->cslot; out.cslot_cap = c->cslot_cap; out.scratch = c->trav_scratch; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
+    out.cslot = c->cslot; out.cslot_cap = c->cslot_cap; out.scratch = c->trav_scratch; out.hit_scratch = c->trav_hit_scratch; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
     uint32_t* wc = c->sort_counters + 8;   // spare counter word
     k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc);
     // persistent grid: two CTAs per SM (shared-memory bound), work handed out through an atomic counter
