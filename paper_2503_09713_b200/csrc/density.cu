@@ -29,7 +29,14 @@ __device__ __forceinline__ double sep_r(double xa, double ya, double za, const d
         if (db.periodic[1]) { if (dy > db.halfL[1]) dy -= db.L[1]; else if (dy < -db.halfL[1]) dy += db.L[1]; }
         if (db.periodic[2]) { if (dz > db.halfL[2]) dz -= db.L[2]; else if (dz < -db.halfL[2]) dz += db.L[2]; }
     }
-    return sqrt(dx * dx + dy * dy + dz * dz);
+    // r = r2 / sqrt(r2) with the hardware reciprocal-square-root seed and one third-order refinement (relative error
+    // ~1e-16, no range checks: r2 is a squared separation); the particle itself (r2 = 0) gives r = 0
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+    const double e = fma(r2, -(y0 * y0), 1.0);
+    const double y = fma(fma(e, 0.375, 0.5), y0 * e, y0);
+    return r2 > 0.0 ? r2 * y : 0.0;
 }
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
