@@ -83,8 +83,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         }
     }
     // sums over the list at smoothing length h: rs = sum m f(q), ss = sum m (3 f + q f')
-    auto sums = [&](double h, double& rho_sum, double& S) {
-        const double hinv = 1.0 / h;
+    auto sums = [&](double hinv, double& rho_sum, double& S) {
         double rs = 0.0, ss = 0.0;
 #pragma unroll
         for (int c = 0; c < kRegChunks; ++c) {
@@ -114,25 +113,26 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         S = -c3 * hinv * ss;          // sum_b m_b dW/dh
     };
 
-    const double inv_lambda = 1.0 / dp.lambda;
+    const double inv_lambda = 1.0 / dp.lambda, h0inv = 1.0 / h0;
     double h = h0;
     bool exceeded = false, converged = false, active = pv;
     int it = 0;
     while (__any_sync(0xffffffffu, active)) {      // the four octets of a warp iterate together
         double rho_sum, S;
-        sums(h, rho_sum, S);
+        const double hinv = 1.0 / h;                                // the one reciprocal of a sweep besides f / f'
+        sums(hinv, rho_sum, S);
         if (active) {
             ++it;
-            const double hf = dp.hfact / h;
+            const double hf = dp.hfact * hinv;
             const double rho_h = ma * hf * hf * hf;                 // F1
             const double f = rho_sum - rho_h;                       // F2
-            const double fp = S + 3.0 * rho_h / h;                  // exact derivative (reading A5)
+            const double fp = S + 3.0 * rho_h * hinv;               // exact derivative (reading A5)
             double hnew = h - f / fp;                               // Alg. 7 l.10
             if (!(fp > 0.0) || (hnew - h) * f > 0.0 || !(hnew == hnew))
                 hnew = (f > 0.0) ? h * inv_lambda : h * dp.lambda;  // safeguard 2b
             if (hnew > h * dp.lambda) hnew = h * dp.lambda;         // Alg. 7 l.11-13
             else if (hnew < h * inv_lambda) hnew = h * inv_lambda;
-            const double eps = fabs(hnew - h) / h0;                 // Alg. 7 l.14
+            const double eps = fabs(hnew - h) * h0inv;              // Alg. 7 l.14
             if (hnew > h0 * dp.chi) { hnew = h0 * dp.chi; exceeded = true; }   // Alg. 7 l.15-17
             h = hnew;
             if (!exceeded && eps <= dp.eps_h) converged = true;
@@ -140,8 +140,9 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         }
     }
     double rho_sum, S;
-    sums(h, rho_sum, S);
-    const double hf = dp.hfact / h;
+    const double hinv = 1.0 / h;
+    sums(hinv, rho_sum, S);
+    const double hf = dp.hfact * hinv;
     const double rho_a = ma * hf * hf * hf;
     out.h = h;
     out.rho = rho_a;
