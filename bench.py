@@ -35,7 +35,7 @@ FLOP_PER_PAIR_FORCE = 93              # Eq. 3-6, 8-10 per pair
 FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair (single pass)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
-# workload (profiles/r1_ncu_all_v20.md); only quoted when bench runs that workload
+# workload (profiles/r1_ncu_all_v22.md); only quoted when bench runs that workload
 NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.55e9, "traverse": 4.51e9, "density": 4.85e9}   # unchanged since v16
 
 
