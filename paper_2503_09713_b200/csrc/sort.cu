@@ -1,7 +1,7 @@
 // sort.cu -- a2: stable LSD radix sort of (key u64, val u32), onesweep style: one upfront histogram of all
 // eight 8-bit digits, then ONE pass per digit that reads each (key,val) once and writes it once; tile prefixes
 // are resolved with a decoupled look-back over single-word (flag|count) status entries; ranking inside a tile
-// uses warp-level __match_any_sync multisplit. Replaces the paper's bitonic sort, which it
+// uses a warp-level ballot multisplit. Replaces the paper's bitonic sort, which it
 // says dominates the tree build. HBM-bound: 8 B + 8 x 24 B = 200 B per particle.
 #include <utility>
 
@@ -127,14 +127,22 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __
         k[i] = (idx < N) ? kin[idx] : ~0ull;
     }
     const unsigned lt = lanemask_lt();
-    // all match masks first (independent MATCH instructions pipeline), then the serial counter updates
+    // all match masks first, then the serial counter updates
     unsigned mm[kItems];
 #pragma unroll
     for (int i = 0; i < kItems; ++i) {
         const bool valid = (wbase + i * 32) < N;
         const unsigned act = __ballot_sync(0xffffffffu, valid);
         const unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
-        mm[i] = valid ? __match_any_sync(act, d) : 0u;
+        // lanes with the same digit: eight ballots, one per digit bit (MATCH.ANY was the kernel's largest stall)
+        unsigned m = valid ? act : 0u;
+#pragma unroll
+        for (int b = 0; b < kRadixBits; ++b) {
+            const bool bit = ((d >> b) & 1u) != 0u;
+            const unsigned bal = __ballot_sync(0xffffffffu, bit);
+            m &= bit ? bal : ~bal;
+        }
+        mm[i] = m;
     }
 #pragma unroll
     for (int i = 0; i < kItems; ++i) {
