@@ -18,6 +18,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kItems = 16;                       // keys per thread
 constexpr int kTile = kSortThreads * kItems;     // 4096 keys per tile
+constexpr int kLookBatch = 4;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
 
 // ---- kernel 1: histograms of all 8 digits in one read of the keys ----
@@ -184,14 +185,25 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __
         // decoupled look-back
         uint32_t excl = 0;
         if (tile > 0) {
+            // four predecessors per round trip (independent loads), consumed in order up to the first one that has
+            // not published yet or carries an inclusive prefix
             int64_t t = (int64_t)tile - 1;
-            for (;;) {
-                uint32_t v = status[(size_t)t * kRadix + d];
-                uint32_t flag = v & ~kValMask;
-                if (flag == 0) continue;              // predecessor has not published yet: spin
-                excl += v & kValMask;
-                if (flag == kFlagIncl) break;
-                --t;
+            for (bool done = false; !done;) {
+                uint32_t v[kLookBatch];
+#pragma unroll
+                for (int j = 0; j < kLookBatch; ++j) {
+                    uint32_t vv = 2u << 30;           // before tile 0: inclusive prefix 0
+                    if (t - j >= 0) vv = status[(size_t)(t - j) * kRadix + d];
+                    v[j] = vv;
+                }
+#pragma unroll
+                for (int j = 0; j < kLookBatch; ++j) {
+                    const uint32_t flag = v[j] & ~kValMask;
+                    if (flag == 0) break;             // not published yet: poll again from this tile
+                    excl += v[j] & kValMask;
+                    --t;
+                    if (flag == kFlagIncl) { done = true; break; }
+                }
             }
             *my = kFlagIncl | (excl + run);
         }
