@@ -19,6 +19,7 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kItems = 16;                       // keys per thread
 constexpr int kTile = kSortThreads * kItems;     // 4096 keys per tile
 constexpr int kLookBatch = 4;
+__device__ __forceinline__ uint32_t pad(uint32_t j) { return j + (j >> 5); }
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
 
 // ---- kernel 1: histograms of all 8 digits in one read of the keys ----
@@ -94,8 +95,8 @@ __global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ gh
 
 // ---- kernel 3: one onesweep pass ----
 struct SortSmem {
-    uint64_t keys[kTile];
-    uint32_t vals[kTile];
+    uint64_t keys[kTile + kTile / 32];       // indexed through pad(): slots a power of two apart (digits of a
+    uint32_t vals[kTile + kTile / 32];       // regular lattice) would otherwise all fall into one bank
     uint32_t whist[kSortWarps][kRadix];
     uint32_t gofs[kRadix];
     uint32_t wsum[kRadix / 32];
@@ -220,19 +221,19 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __
         if (idx < N) {
             unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
             uint32_t slot = s.whist[w][d] + rank[i];
-            s.keys[slot] = k[i];
-            s.vals[slot] = vin[idx];
+            s.keys[pad(slot)] = k[i];
+            s.vals[pad(slot)] = vin[idx];
         }
     }
     __syncthreads();
 
     // coalesced runs out to global memory
     for (int j = tid; j < tile_n; j += kSortThreads) {
-        uint64_t kk = s.keys[j];
+        uint64_t kk = s.keys[pad((uint32_t)j)];
         unsigned d = (unsigned)(kk >> shift) & (kRadix - 1);
         uint32_t pos = s.gofs[d] + (uint32_t)j;
         kout[pos] = kk;
-        vout[pos] = s.vals[j];
+        vout[pos] = s.vals[pad((uint32_t)j)];
     }
 }
 
