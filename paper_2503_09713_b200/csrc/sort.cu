@@ -14,9 +14,9 @@ constexpr int kRadix = 1 << kRadixBits;
 constexpr int kPasses = 8;
 constexpr int kPrefixPass = 3;                   // prefix mode sorts on digits 3..7 = bits 24..63 (40 bits)
 constexpr int kPrefixShift = kPrefixPass * 8;
-constexpr int kSortThreads = 256;
+constexpr int kSortThreads = 512;
 constexpr int kSortWarps = kSortThreads / 32;
-constexpr int kItems = 16;                       // keys per thread
+constexpr int kItems = 8;                        // keys per thread
 constexpr int kTile = kSortThreads * kItems;     // 4096 keys per tile
 constexpr int kLookBatch = 4;
 __device__ __forceinline__ uint32_t pad(uint32_t j) { return j + (j >> 5); }
@@ -161,26 +161,28 @@ __global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __
     __syncthreads();
 
     // per digit (thread d): exclusive scan over the warps, tile count, look-back, tile-local digit start
-    {
-        const unsigned d = tid;
-        uint32_t run = 0;
+    const unsigned d = tid;
+    uint32_t run = 0, inc = 0;
+    volatile uint32_t* my = status + (size_t)tile * kRadix + d;
+    if (tid < kRadix) {
 #pragma unroll
         for (int ww = 0; ww < kSortWarps; ++ww) {
             uint32_t t = s.whist[ww][d];
             s.whist[ww][d] = run;
             run += t;
         }
-        volatile uint32_t* my = status + (size_t)tile * kRadix + d;
         *my = (tile == 0 ? kFlagIncl : kFlagAgg) | run;
         // tile-local exclusive scan of the 256 digit counts
-        uint32_t inc = run;
+        inc = run;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
             if (lane >= (unsigned)o) inc += t;
         }
         if (lane == 31) s.wsum[w] = inc;
-        __syncthreads();
+    }
+    __syncthreads();
+    if (tid < kRadix) {
         uint32_t dstart = inc - run;
         for (unsigned j = 0; j < w; ++j) dstart += s.wsum[j];
         // decoupled look-back
