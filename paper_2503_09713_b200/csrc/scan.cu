@@ -44,23 +44,34 @@ __global__ void __launch_bounds__(kScanThreads) k_scan(const uint32_t* __restric
         if (j < w) wbase += wsum[j];
         agg += wsum[j];
     }
-    if (tid == 0) {
+    if (w == 0) {
+        // look-back by one warp: 32 predecessors per round trip; the lanes up to the nearest inclusive prefix must all
+        // have published before their values are summed
         volatile uint64_t* my = status + tile;
-        *my = (tile == 0 ? kSFlagIncl : kSFlagAgg) | agg;
+        if (lane == 0) *my = (tile == 0 ? kSFlagIncl : kSFlagAgg) | agg;
         uint64_t excl = 0;
         if (tile > 0) {
             int64_t t = (int64_t)tile - 1;
             for (;;) {
-                uint64_t sv = status[t];
-                uint64_t flag = sv & ~kSValMask;
-                if (flag == 0) continue;          // spin: predecessor tiles are always already running
-                excl += sv & kSValMask;
-                if (flag == kSFlagIncl) break;
-                --t;
+                const int64_t idx = t - (int64_t)lane;
+                uint64_t sv = 2ull << 62;                                   // before tile 0: inclusive prefix 0
+                if (idx >= 0) sv = status[idx];
+                const unsigned flag = (unsigned)(sv >> 62);
+                const unsigned not_ready = __ballot_sync(0xffffffffu, flag == 0u);
+                const unsigned incl = __ballot_sync(0xffffffffu, flag == 2u);
+                const unsigned first = incl ? (unsigned)__ffs(incl) - 1u : 31u;
+                const unsigned need = (first == 31u) ? 0xffffffffu : ((2u << first) - 1u);
+                if (not_ready & need) continue;                             // poll again
+                uint64_t val = (lane <= first) ? (sv & kSValMask) : 0ull;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
+                excl += val;
+                if (incl) break;
+                t -= 32;
             }
-            *my = kSFlagIncl | (excl + agg);
+            if (lane == 0) *my = kSFlagIncl | (excl + agg);
         }
-        s_excl = excl;
+        if (lane == 0) s_excl = excl;
     }
     __syncthreads();
     uint64_t run = s_excl + wbase + inc - tsum;
