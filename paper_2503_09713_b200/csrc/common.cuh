@@ -218,6 +218,8 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 // M4 cubic B-spline f(q) and f'(q) (reading O6); branch-light form.
 __device__ __forceinline__ void m4(double q, double& f, double& df);
+// max(a, 0) by the sign bit (integer pipe): a = +-0 gives 0 either way
+__device__ __forceinline__ double clamp_pos(double a) { return __double2hiint(a) >= 0 ? a : 0.0; }
 // f(q) and f'(q) of kernel K. M5 and M6 in clamped-power form: f = sum_i c_i (a_i - q)_+^p
 template <int K>
 __device__ __forceinline__ void kern_f_df(double q, double& f, double& df) {
@@ -225,13 +227,13 @@ __device__ __forceinline__ void kern_f_df(double q, double& f, double& df) {
         m4(q, f, df);
     } else if (K == 1) {
         const double a = 2.5 - q, b = 1.5 - q, c = 0.5 - q;
-        const double t1 = a > 0.0 ? a : 0.0, t2 = b > 0.0 ? b : 0.0, t3 = c > 0.0 ? c : 0.0;
+        const double t1 = clamp_pos(a), t2 = clamp_pos(b), t3 = clamp_pos(c);
         const double c1 = t1 * t1 * t1, c2 = t2 * t2 * t2, c3 = t3 * t3 * t3;
         f = fma(10.0 * c3, t3, fma(-5.0 * c2, t2, c1 * t1));
         df = -4.0 * fma(10.0, c3, fma(-5.0, c2, c1));
     } else {
         const double a = 3.0 - q, b = 2.0 - q, c = 1.0 - q;
-        const double t1 = a > 0.0 ? a : 0.0, t2 = b > 0.0 ? b : 0.0, t3 = c > 0.0 ? c : 0.0;
+        const double t1 = clamp_pos(a), t2 = clamp_pos(b), t3 = clamp_pos(c);
         const double s1 = t1 * t1, s2 = t2 * t2, s3 = t3 * t3;
         const double q1 = s1 * s1, q2 = s2 * s2, q3 = s3 * s3;
         f = fma(15.0 * q3, t3, fma(-6.0 * q2, t2, q1 * t1));
@@ -244,7 +246,10 @@ __device__ __forceinline__ void m4(double q, double& f, double& df) {
     double dfo = -0.75 * t2 * t2;
     double fi = 1.0 + q * q * (0.75 * q - 1.5);   // inner branch q < 1
     double dfi = q * (2.25 * q - 3.0);
-    bool in = q < 1.0, sup = q < 2.0;
+    // q >= +0: doubles order as their bit patterns, so the two range tests are integer compares of the high word
+    // (exactly q < 1, q < 2) and stay off the FP64 pipe
+    const int qh = __double2hiint(q);
+    bool in = qh < 0x3FF00000, sup = qh < 0x40000000;
     f = in ? fi : (sup ? fo : 0.0);
     df = in ? dfi : (sup ? dfo : 0.0);
 }
