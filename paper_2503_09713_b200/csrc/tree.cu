@@ -7,36 +7,38 @@
 
 namespace sph {
 
-__device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int64_t N, uint64_t ki, int64_t i, int64_t j) {
-    if (j < 0 || j >= N) return -1;
+// indices are 32-bit: N < 2^30 (sph_init_ex), and i + lmax * d stays within (-2^30, 2^31 - 2]
+__device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int N, uint64_t ki, int i, int j) {
+    if ((unsigned)j >= (unsigned)N) return -1;
     uint64_t kj = __ldg(key + j);
     if (ki != kj) return __clzll((long long)(ki ^ kj));
-    return 64 + __clz((int)((uint32_t)i ^ (uint32_t)j));
+    return 64 + __clz(i ^ j);
 }
 
 // one thread per internal node i in [0, N-2]
-__global__ void __launch_bounds__(256) k_karras(int64_t N, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
+__global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
                                                 int32_t* __restrict__ parent, uint32_t* __restrict__ gflag) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int N = (int)N64;
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
     if (i >= N - 1) return;
     const uint64_t ki = key[i];
     const int dn = delta_aug(key, N, ki, i, i + 1), dp = delta_aug(key, N, ki, i, i - 1);
-    const int64_t d = (dn - dp) > 0 ? 1 : -1;
+    const int d = (dn - dp) > 0 ? 1 : -1;
     const int dmin = (d > 0) ? dp : dn;
-    int64_t lmax = 2;
+    int lmax = 2;
     while (delta_aug(key, N, ki, i, i + lmax * d) > dmin) lmax <<= 1;
-    int64_t l = 0;
-    for (int64_t t = lmax >> 1; t >= 1; t >>= 1)
+    int l = 0;
+    for (int t = lmax >> 1; t >= 1; t >>= 1)
         if (delta_aug(key, N, ki, i, i + (l + t) * d) > dmin) l += t;
-    const int64_t j = i + l * d;
+    const int j = i + l * d;
     const int dnode = delta_aug(key, N, ki, i, j);
-    int64_t s = 0, t = l;
+    int s = 0, t = l;
     do {
         t = (t + 1) >> 1;
         if (delta_aug(key, N, ki, i, i + (s + t) * d) > dnode) s += t;
     } while (t > 1);
-    const int64_t gamma = i + s * d + (d < 0 ? -1 : 0);
-    const int64_t lo = min(i, j), hi = max(i, j);
+    const int gamma = i + s * d + (d < 0 ? -1 : 0);
+    const int lo = min(i, j), hi = max(i, j);
     nodes[i].other = (int32_t)j;
     nodes[i].split = (int32_t)gamma;
     parent[(lo == gamma) ? (N - 1 + gamma) : gamma] = (int32_t)i;
