@@ -55,6 +55,29 @@ __device__ __forceinline__ double octet_sum(double v) {
 }
 
 struct DensPar { double hfact, chi, lambda, eps_h; int max_iter; };
+
+// f(q) and g(q) = (3 f + q f') / kGScale of kernel K: what a sweep sums (dW/dh = -C h^-4 (3 f + q f')). For M4 the two
+// polynomials of each branch are evaluated directly (14 instead of 16 FP64 instructions per neighbour and sweep):
+//   q < 1:      f = 1 + q^2 (3q/4 - 3/2),   g = 1 + q^2 (3q/2 - 5/2)
+//   1 <= q < 2: f = (2-q)^3 / 4,            g = (2-q)^2 (2 - 2q) / 4          (g = (3 f + q f') / 3)
+template <int K> constexpr double kGScale = (K == 0) ? 3.0 : 1.0;
+template <int K>
+__device__ __forceinline__ void kern_f_g(double q, double& f, double& g) {
+    if (K == 0) {
+        const double q2 = q * q, t = 2.0 - q;
+        const double fi = fma(q2, fma(0.75, q, -1.5), 1.0), gi = fma(q2, fma(1.5, q, -2.5), 1.0);
+        const double b = 0.25 * (t * t);
+        const double fo = b * t, go = b * (t - q);
+        const int qh = __double2hiint(q);                        // q >= +0: integer range tests, see m4()
+        const bool in = qh < 0x3FF00000, sup = qh < 0x40000000;
+        f = in ? fi : (sup ? fo : 0.0);
+        g = in ? gi : (sup ? go : 0.0);
+    } else {
+        double df;
+        kern_f_df<K>(q, f, df);
+        g = fma(q, df, 3.0 * f);
+    }
+}
 struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 
 // UNIM: every candidate of the group has the same mass (checked while staging): the mass factors out of the sums
@@ -87,30 +110,30 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         double rs = 0.0, ss = 0.0;
 #pragma unroll
         for (int c = 0; c < kRegChunks; ++c) {
-            double qq = r[c] * hinv, f, df;
-            kern_f_df<K>(qq, f, df);
+            double f, g;
+            kern_f_g<K>(r[c] * hinv, f, g);
             if (UNIM) {
                 rs += f;
-                ss += fma(qq, df, 3.0 * f);
+                ss += g;
             } else {
                 rs = fma(mb[c], f, rs);
-                ss = fma(mb[c], fma(qq, df, 3.0 * f), ss);
+                ss = fma(mb[c], g, ss);
             }
         }
         for (int k = kRegChunks * 8 + (int)sl; k < n; k += 8) {      // long lists: re-gather from smem
             uint32_t b = li[k];
             if (GLOB) b = cs[b];
-            double qq = sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, df;
+            double f, g;
             const double mm = UNIM ? 1.0 : sm[b];
-            kern_f_df<K>(qq, f, df);
+            kern_f_g<K>(sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, g);
             rs = fma(mm, f, rs);
-            ss = fma(mm, fma(qq, df, 3.0 * f), ss);
+            ss = fma(mm, g, ss);
         }
         rs = octet_sum(rs);
         ss = octet_sum(ss);
         const double c3 = (UNIM ? m0 : 1.0) * kern_cnorm(K) * hinv * hinv * hinv;
         rho_sum = c3 * rs;            // Eq. 1-2
-        S = -c3 * hinv * ss;          // sum_b m_b dW/dh
+        S = -c3 * hinv * (kGScale<K> * ss);   // sum_b m_b dW/dh
     };
 
     const double inv_lambda = 1.0 / dp.lambda, h0inv = 1.0 / h0;
