@@ -129,7 +129,9 @@ __device__ __forceinline__ void record_hit(GroupCtx& G, uint32_t& wp, uint32_t l
     } else {
         // wp = 32-bit shared-memory address of the lane's next free entry; the row has kHitSlack entries
         // beyond kHitCap, so no capacity check is needed inside a bucket
-        asm volatile("st.shared.u16 [%0], %1;" :: "r"(wp), "h"((unsigned short)local) : "memory");
+        // no "memory" clobber: the hit rows alias nothing that is read inside a bucket's test loop, and the loads of
+        // the next candidates must be free to move above this store (stage2 closes the loop with a compiler barrier)
+        asm volatile("st.shared.u16 [%0], %1;" :: "r"(wp), "h"((unsigned short)local));
         wp += 2u;
     }
 }
@@ -189,12 +191,16 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             for (uint32_t ci = 0; ci < nk4; ci += 4) {
                 const uint4 id4 = *reinterpret_cast<const uint4*>(&s.cid[ci]);
                 const uint32_t ids[4] = {id4.x, id4.y, id4.z, id4.w};
+                // all four candidates are loaded before the first hit is stored: the assembler keeps shared-memory
+                // loads behind earlier shared-memory stores, which would serialise the four tests
+                double2 a[4], c[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { a[u] = s.cxy[ci + u]; c[u] = s.czr[ci + u]; }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const double2 a = s.cxy[ci + u], c = s.czr[ci + u];
-                    const double dx = __dsub_rn(G.xq, a.x), dy = __dsub_rn(G.yq, a.y), dz = __dsub_rn(G.zq, c.x);
+                    const double dx = __dsub_rn(G.xq, a[u].x), dy = __dsub_rn(G.yq, a[u].y), dz = __dsub_rn(G.zq, c[u].x);
                     const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                    if (lt_either(d2, G.rc2q, c.y)) record_hit<DIRECT>(G, wp, ids[u]);
+                    if (lt_either(d2, G.rc2q, c[u].y)) record_hit<DIRECT>(G, wp, ids[u]);
                 }
             }
         } else {
@@ -207,6 +213,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                 if (lt_either(d2, G.rc2q, c.y)) record_hit<DIRECT>(G, wp, s.cid[ci]);
             }
         }
+        asm volatile("" ::: "memory");                    // the row stores above are done as far as the compiler knows
         if (!DIRECT) {
             const uint32_t got = (wp - w0) >> 1;
             G.nhit += got;
