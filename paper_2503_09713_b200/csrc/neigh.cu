@@ -37,7 +37,7 @@ constexpr int kStackSlack = 192;         // above kStackCap - kStackSlack the wa
 constexpr int kPendCap = 64;             // candidate buckets buffered before stage 2 runs
 constexpr int kHitCap = 112;             // buffered hits per lane
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
-constexpr int kHitStride = kHitCap + kHitSlack + 2;   // in u16: 73 words per lane row (odd: rows start in distinct banks)
+constexpr int kHitStride = kHitCap + kHitSlack + 4;   // in u16: 296 B per lane row (8-byte aligned: copied out as u64)
 constexpr int kShare = 4;               // consecutive groups that share one tree walk
 constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
 constexpr int kSpillCap = 512;            // hits per lane that can spill from the shared-memory row to the warp's global scratch
@@ -469,26 +469,27 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
         // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and candidate slots ----
-        const uint32_t nhit = qv ? G.nhit : 0u;
+        // every particle's list starts at a multiple of four entries (8 B), so that rows are copied out as u64
+        const uint32_t nhit = qv ? G.nhit : 0u, nhit4 = (nhit + 3u) & ~3u;
         const uint32_t nc = G.ncs, nc4 = (nc + 3u) & ~3u;
-        uint32_t incl = nhit;
+        uint32_t incl = nhit4;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
             if (lane >= (unsigned)o) incl += t;
         }
-        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31), total_exact = __reduce_add_sync(0xffffffffu, nhit);
         unsigned long long lbase = 0, bbase = 0;
         if (lane == 0) {
             lbase = atomicAdd(&sc->list_cursor, (unsigned long long)((total + 7u) & ~7u));
             bbase = atomicAdd(&sc->cslot_cursor, (unsigned long long)nc4);
-            atomicAdd(&sc->n_neigh, (unsigned long long)total);
+            atomicAdd(&sc->n_neigh, (unsigned long long)total_exact);
         }
         lbase = __shfl_sync(0xffffffffu, lbase, 0);
         bbase = __shfl_sync(0xffffffffu, bbase, 0);
         const bool fits = (lbase + ((total + 7u) & ~7u) <= out.list_cap) && (bbase + nc4 <= out.cslot_cap) &&
                           ((uint64_t)g < out.ginfo_cap) && (nc <= 65535u);
-        const uint64_t my_start = lbase + (incl - nhit);
+        const uint64_t my_start = lbase + (incl - nhit4);
         if (qv) {
             out.cnt[a] = nhit;
             out.lstart[a] = my_start;
@@ -508,16 +509,19 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                 const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
                 for (uint32_t p = 0; p < nq; ++p) {
                     const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
-                    uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - np);
-                    uint32_t nrow = np;
+                    uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 3u) & ~3u));
                     if (spilled) {
                         const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p);
                         const uint16_t* src = hit_row + (size_t)p * kSpillCap;
                         for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
                         sp0 += ns;
-                        nrow = np - ns;
+                        for (uint32_t k = lane; k < np - ns; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
+                    } else {
+                        // four entries per lane and store (the up to three entries of padding are never read)
+                        const uint64_t* src = reinterpret_cast<const uint64_t*>(&s.hits[p * kHitStride]);
+                        uint64_t* dst = reinterpret_cast<uint64_t*>(out.lists + sp0);
+                        for (uint32_t k = lane; k < (np + 3u) >> 2; k += 32) dst[k] = src[k];
                     }
-                    for (uint32_t k = lane; k < nrow; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
                 }
             } else {
                 // fallback: second walk writing directly at the now-known positions
