@@ -504,7 +504,11 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             const bool overflow = G.hard_overflow || (nc > (uint32_t)kScrCap);
             if (!overflow) {
                 __syncwarp();
-                for (uint32_t j = lane; j < nc; j += 32) out.cslot[bbase + j] = scr_row[j];
+                {   // candidate slots, four per lane and copy (both sides 16-byte aligned; the padding is never read)
+                    const uint4* src = reinterpret_cast<const uint4*>(scr_row);
+                    uint4* dst = reinterpret_cast<uint4*>(out.cslot + bbase);
+                    for (uint32_t j = lane; j < (nc4 >> 2); j += 32) dst[j] = src[j];
+                }
                 // lists: the warp copies one particle's buffered list at a time (coalesced 16-bit stores)
                 const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
                 for (uint32_t p = 0; p < nq; ++p) {
