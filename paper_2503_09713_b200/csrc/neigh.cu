@@ -204,13 +204,21 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                 }
             }
         } else {
-            for (uint32_t ci = 0; ci < nk; ++ci) {
-                const double2 a = s.cxy[ci], c = s.czr[ci];
-                const double dx = min_image(__dsub_rn(G.xq, a.x), tb.L[0], tb.halfL[0], tb.periodic[0]);
-                const double dy = min_image(__dsub_rn(G.yq, a.y), tb.L[1], tb.halfL[1], tb.periodic[1]);
-                const double dz = min_image(__dsub_rn(G.zq, c.x), tb.L[2], tb.halfL[2], tb.periodic[2]);
-                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                if (lt_either(d2, G.rc2q, c.y)) record_hit<DIRECT>(G, wp, s.cid[ci]);
+            // same grouping; the padding candidates sit at 1e300, whose minimum image is still out of reach
+            for (uint32_t ci = 0; ci < nk4; ci += 4) {
+                const uint4 id4 = *reinterpret_cast<const uint4*>(&s.cid[ci]);
+                const uint32_t ids[4] = {id4.x, id4.y, id4.z, id4.w};
+                double2 a[4], c[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { a[u] = s.cxy[ci + u]; c[u] = s.czr[ci + u]; }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const double dx = min_image(__dsub_rn(G.xq, a[u].x), tb.L[0], tb.halfL[0], tb.periodic[0]);
+                    const double dy = min_image(__dsub_rn(G.yq, a[u].y), tb.L[1], tb.halfL[1], tb.periodic[1]);
+                    const double dz = min_image(__dsub_rn(G.zq, c[u].x), tb.L[2], tb.halfL[2], tb.periodic[2]);
+                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    if (lt_either(d2, G.rc2q, c[u].y)) record_hit<DIRECT>(G, wp, ids[u]);
+                }
             }
         }
         asm volatile("" ::: "memory");                    // the row stores above are done as far as the compiler knows
