@@ -77,13 +77,15 @@ struct TravOut {
 // about six instructions on sm_100
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+// max(a, 0) by the sign bit (integer pipe; `a > 0 ? a : 0` compiles to a NaN-quieting fp64 max of six instructions)
+__device__ __forceinline__ double clamp0(double a) { return __double2hiint(a) >= 0 ? a : 0.0; }
 
 // separation of two intervals [alo,ahi], [blo,bhi] along one axis (0 if they overlap), minimum over periodic images
 __device__ __forceinline__ double axis_gap(double alo, double ahi, double blo, double bhi, double L, int periodic) {
-    double g = dmax(dmax(blo - ahi, alo - bhi), 0.0);
+    double g = clamp0(dmax(blo - ahi, alo - bhi));
     if (periodic) {
-        g = dmin(g, dmax(blo + L - ahi, 0.0));
-        g = dmin(g, dmax(alo - bhi + L, 0.0));
+        g = dmin(g, clamp0(blo + L - ahi));
+        g = dmin(g, clamp0(alo - bhi + L));
     }
     return g;
 }
@@ -165,9 +167,9 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
         // Buckets that may wrap keep every candidate.
         bool keep = lane < bn;
         if (keep && !wrap) {
-            const double gx = dmax(dmax(G.gxl - cx, cx - G.gxh), 0.0);
-            const double gy = dmax(dmax(G.gyl - cy, cy - G.gyh), 0.0);
-            const double gz = dmax(dmax(G.gzl - cz, cz - G.gzh), 0.0);
+            const double gx = clamp0(dmax(G.gxl - cx, cx - G.gxh));
+            const double gy = clamp0(dmax(G.gyl - cy, cy - G.gyh));
+            const double gz = clamp0(dmax(G.gzl - cz, cz - G.gzh));
             keep = gx * gx + gy * gy + gz * gz <= dmax(rc2, G.rc2g) * (1.0 + 1e-9);
         }
         const unsigned km = __ballot_sync(0xffffffffu, keep);
