@@ -79,7 +79,9 @@ typedef struct {
                            acceleration is recalculated with v* <- v^{n+1} and the correction applied again   */
   double lambda_stiff;  /* 2.0  stiffness of the CFL multiplier relaxation (value not given in the paper)        */
   int32_t max_recycle;  /* 10   cap on re-cycles per step                                                        */
-  int32_t reserved2;
+  int32_t group_max;    /* 32   particles per leaf group / traversal bucket, 1..32 (0 = 32): the paper's particles-per-
+                           leaf knob of the leaf reduction (Fig. 16). Results do
+                           not depend on it (the neighbour sets are exact for any grouping); the speed does           */
 } sph_params;
 
 /* Device-memory hooks so that the host framework (PyTorch's caching allocator) owns device memory.

@@ -49,6 +49,7 @@ struct TravBox {
     double L[3], halfL[3];
     int periodic[3];
     double gg_pad;                       // absolute slack added to the conservative box test
+    uint32_t gmax;                       // nodes with <= gmax particles are buckets (sph_params.group_max)
 };
 
 struct TravWarpSmem {
@@ -272,7 +273,7 @@ __device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, cons
         r.split = (uint32_t)(ints >> 32);
         r.rlo = min(e, (uint32_t)other);
         r.rhi = max(e, (uint32_t)other);
-        r.small = (r.rhi - r.rlo + 1) <= (uint32_t)kGroup;
+        r.small = (r.rhi - r.rlo + 1) <= tb.gmax;
     }
     const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
     const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
@@ -590,6 +591,7 @@ int launch_traverse(sph_ctx* c) {
         Lmax = fmax(Lmax, tb.L[k]);
     }
     tb.gg_pad = 1e-14 * Lmax;
+    tb.gmax = (uint32_t)c->p.group_max;
     const double rk_chi = kern_radius(c->p.kernel) * c->p.chi;
     TravOut out;
     out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;

@@ -17,7 +17,7 @@ __device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int N
 
 // one thread per internal node i in [0, N-2]
 __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
-                                                int32_t* __restrict__ parent, uint32_t* __restrict__ gflag) {
+                                                int32_t* __restrict__ parent, uint32_t* __restrict__ gflag, int gmax) {
     const int N = (int)N64;
     const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
     if (i >= N - 1) return;
@@ -44,12 +44,12 @@ __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __r
     parent[(lo == gamma) ? (N - 1 + gamma) : gamma] = (int32_t)i;
     parent[(hi == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1)] = (int32_t)i;
     if (i == 0) parent[0] = -1;
-    // leaf groups: children of nodes with more than kGroup particles that themselves hold <= kGroup
-    if (hi - lo + 1 <= kGroup) {
+    // leaf groups: children of nodes with more than gmax (sph_params.group_max <= kGroup) particles that themselves hold <= gmax
+    if (hi - lo + 1 <= gmax) {
         if (i == 0) gflag[0] = 1u;   // the whole tree is one group
     } else {
-        if (gamma - lo + 1 <= kGroup) gflag[lo] = 1u;        // left child covers [lo, gamma]
-        if (hi - gamma <= kGroup) gflag[gamma + 1] = 1u;     // right child covers [gamma + 1, hi]
+        if (gamma - lo + 1 <= gmax) gflag[lo] = 1u;        // left child covers [lo, gamma]
+        if (hi - gamma <= gmax) gflag[gamma + 1] = 1u;     // right child covers [gamma + 1, hi]
     }
 }
 
@@ -197,7 +197,7 @@ int launch_tree(sph_ctx* c) {
     const int64_t N = c->N;
     SPH_CUDA(c, cudaMemsetAsync(c->gflag, 0, (size_t)N * sizeof(uint32_t), c->stream));
     if (N >= 2) {
-        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag);
+        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag, c->p.group_max);
         c->launches++;
     } else {
         k_single_group<<<1, 1, 0, c->stream>>>(c->gflag);

@@ -641,3 +641,18 @@ def test_c3_disc_full_size_sampled_parity():
     cnt_orig[perm] = np.diff(offs).astype(np.int64)
     assert np.array_equal(cnt_orig[tgt_g], np.diff(oo).astype(np.int64)[tgt])
     sim.close()
+
+
+@pytest.mark.parametrize("gmax", [1, 5, 8, 16])
+def test_group_max_sweep_is_exact(gmax):
+    """sph_params.group_max (the paper's particles-per-leaf knob, Fig. 16): every stage stays in parity
+    with the oracle for any leaf-group / bucket size; only the number of groups changes."""
+    from paper_2503_09713_b200 import binding as B
+    for w in (W.random_cloud(3000, seed=11), W.sod(16, 12)):
+        sim = _sim(w, params=B.params_for(w, group_max=gmax))
+        _stage_parity(w, sim)
+        st = sim.stats()
+        assert st["n_groups"] >= (w.n + gmax - 1) // gmax
+        sim.step_leapfrog(); sim.step_leapfrog()
+        _invariants(w, sim)
+        sim.close()
