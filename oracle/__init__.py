@@ -157,7 +157,7 @@ def aabb(t, pos_sorted, h_sorted):
 
 
 def set_kernel(k: int = 0):
-    """Select the SPH kernel of every later oracle call: 0 = M4, 1 = M5, 2 = M6 (file-level selector in the C++)."""
+    """Select the SPH kernel of every later oracle call: 0 = M4, 1 = M5, 2 = M6, 3/4/5 = Wendland C2/C4/C6 (file-level selector in the C++)."""
     lib().orc_set_kernel(C.c_int32(int(k)))
 
 

@@ -53,7 +53,7 @@ struct orc_params {
     double eps_v;        // leapfrog corrector check G7: 1e-2 in the paper; 0 disables (reading A15)
     double lambda_stiff; // stiffness of the CFL multiplier G10; value not given, reading A16
     int32_t max_recycle; // cap on corrector re-cycles per step
-    int32_t kernel;      // 0 = M4, 1 = M5, 2 = M6 (informational here: the selector is orc_set_kernel)
+    int32_t kernel;      // 0 = M4, 1 = M5, 2 = M6, 3-5 = Wendland C2, C4, C6 (informational here: the selector is orc_set_kernel)
 };
 
 }  // extern "C"
@@ -65,15 +65,26 @@ namespace {
 // forms, q = r/h, 3-D normalisations 1/pi, 1/(20 pi), 1/(120 pi), support radii 2, 2.5, 3.
 // The kernel in use is a file-level selector set through orc_set_kernel (test infrastructure, single-threaded);
 // 0 = M4 (default), 1 = M5, 2 = M6.
+// Wendland (1995) functions C2, C4, C6 (also named at PAPER.md:43, not printed either), 3 = C2, 4 = C4, 5 = C6: the 3-D
+// forms on the support radius 2h, with t = 1 - q/2,
+//   C2: f = t^4 (1 + 2q),                      C_norm = 21 / (16 pi)
+//   C4: f = t^6 (1 + 3q + 35/12 q^2),          C_norm = 495 / (256 pi)
+//   C6: f = t^8 (1 + 4q + 25/4 q^2 + 4 q^3),   C_norm = 1365 / (512 pi)
+// (pins in tests/test_oracle_sph.py: unit volume integral, f(0) = 1, f' against finite differences of W.)
 int g_kernel = 0;
-#define kRkern (g_kernel == 0 ? 2.0 : g_kernel == 1 ? 2.5 : 3.0)
-#define kCnorm (g_kernel == 0 ? 0.31830988618379067154 : g_kernel == 1 ? 0.31830988618379067154 / 20.0 : 0.31830988618379067154 / 120.0)
+#define kRkern (g_kernel == 1 ? 2.5 : g_kernel == 2 ? 3.0 : 2.0)
+#define kInvPi 0.31830988618379067154
+#define kCnorm (g_kernel == 0 ? kInvPi : g_kernel == 1 ? kInvPi / 20.0 : g_kernel == 2 ? kInvPi / 120.0 : \
+                g_kernel == 3 ? kInvPi * 21.0 / 16.0 : g_kernel == 4 ? kInvPi * 495.0 / 256.0 : kInvPi * 1365.0 / 512.0)
 
 inline double pw(double x, int n) { double r = 1.0; for (int i = 0; i < n; ++i) r *= x; return x > 0.0 ? r : 0.0; }
 
 inline double f_m4(double q) {          // f(q) of the selected kernel (name kept from the M4-only version)
     if (g_kernel == 1) return pw(2.5 - q, 4) - 5.0 * pw(1.5 - q, 4) + 10.0 * pw(0.5 - q, 4);
     if (g_kernel == 2) return pw(3.0 - q, 5) - 6.0 * pw(2.0 - q, 5) + 15.0 * pw(1.0 - q, 5);
+    if (g_kernel == 3) return pw(1.0 - 0.5 * q, 4) * (1.0 + 2.0 * q);
+    if (g_kernel == 4) return pw(1.0 - 0.5 * q, 6) * (1.0 + 3.0 * q + 35.0 / 12.0 * q * q);
+    if (g_kernel == 5) return pw(1.0 - 0.5 * q, 8) * (1.0 + 4.0 * q + 6.25 * q * q + 4.0 * q * q * q);
     if (q < 1.0) return 1.0 - 1.5 * q * q + 0.75 * q * q * q;
     if (q < 2.0) { double t = 2.0 - q; return 0.25 * t * t * t; }
     return 0.0;
@@ -81,6 +92,11 @@ inline double f_m4(double q) {          // f(q) of the selected kernel (name kep
 inline double df_m4(double q) {         // f'(q)
     if (g_kernel == 1) return -4.0 * (pw(2.5 - q, 3) - 5.0 * pw(1.5 - q, 3) + 10.0 * pw(0.5 - q, 3));
     if (g_kernel == 2) return -5.0 * (pw(3.0 - q, 4) - 6.0 * pw(2.0 - q, 4) + 15.0 * pw(1.0 - q, 4));
+    // product rule on t^n p(q), dt/dq = -1/2
+    if (g_kernel == 3) return -2.0 * pw(1.0 - 0.5 * q, 3) * (1.0 + 2.0 * q) + 2.0 * pw(1.0 - 0.5 * q, 4);
+    if (g_kernel == 4) return -3.0 * pw(1.0 - 0.5 * q, 5) * (1.0 + 3.0 * q + 35.0 / 12.0 * q * q) + pw(1.0 - 0.5 * q, 6) * (3.0 + 35.0 / 6.0 * q);
+    if (g_kernel == 5) return -4.0 * pw(1.0 - 0.5 * q, 7) * (1.0 + 4.0 * q + 6.25 * q * q + 4.0 * q * q * q) +
+                              pw(1.0 - 0.5 * q, 8) * (4.0 + 12.5 * q + 12.0 * q * q);
     if (q < 1.0) return -3.0 * q + 2.25 * q * q;
     if (q < 2.0) { double t = 2.0 - q; return -0.75 * t * t; }
     return 0.0;
@@ -194,7 +210,7 @@ inline void eos(const orc_params& p, double rho, double u, double x, double y, d
 extern "C" {
 
 // ---- exported scalar kernel functions (pins: quadrature, continuity, W(0)) ----
-void orc_set_kernel(int32_t k) { g_kernel = (k == 1 || k == 2) ? k : 0; }
+void orc_set_kernel(int32_t k) { g_kernel = (k >= 1 && k <= 5) ? k : 0; }
 double orc_f(double q) { return f_m4(q); }
 double orc_df(double q) { return df_m4(q); }
 double orc_W(double r, double h) { return W(r, h); }

@@ -85,9 +85,12 @@ def test_group_criterion_is_conservative():
 # ---------------------------------------------------------------- kernel (O6)
 
 @pytest.mark.parametrize("kernel,radius,f0,cnorm", [(0, 2.0, 1.0, 1.0 / math.pi), (1, 2.5, 14.375, 1.0 / (20.0 * math.pi)),
-                                                     (2, 3.0, 66.0, 1.0 / (120.0 * math.pi))], ids=["M4", "M5", "M6"])
+                                                     (2, 3.0, 66.0, 1.0 / (120.0 * math.pi)),
+                                                     (3, 2.0, 1.0, 21.0 / (16.0 * math.pi)), (4, 2.0, 1.0, 495.0 / (256.0 * math.pi)),
+                                                     (5, 2.0, 1.0, 1365.0 / (512.0 * math.pi))],
+                         ids=["M4", "M5", "M6", "WendlandC2", "WendlandC4", "WendlandC6"])
 def test_kernel_closed_forms(kernel, radius, f0, cnorm):
-    """B-spline kernels M4, M5, M6: unit volume integral (pins the 3-D normalisations 1/pi, 1/(20 pi),
+    """B-spline kernels M4, M5, M6 and Wendland functions C2, C4, C6: unit volume integral (pins the 3-D normalisations 1/pi, 1/(20 pi),
     1/(120 pi)), closed-form central values (1, 115/8, 66), compact support, continuity of f and f' at the knots,
     F and dW/dh against finite differences of W."""
     L = O.lib()
@@ -449,3 +452,32 @@ def test_corrector_recycle_pins():
         m = 0.5 * m if r > 0 else (1.0 + 2.0 * m) / 3.0
         assert mult == pytest.approx(m, rel=1e-15)
     assert any(r > 0 for r, _ in rec) and any(r == 0 for r, _ in rec)
+
+
+@pytest.mark.parametrize("kernel", [3, 4, 5], ids=["WendlandC2", "WendlandC4", "WendlandC6"])
+def test_wendland_factored_derivative_lattice_and_conservation(kernel):
+    """Wendland C2/C4/C6: f' in its factored closed form (-5 q t^3, -(7/3) q t^5 (2 + 5q),
+    -(11/4) q t^7 (2 + 7q + 8q^2), t = 1 - q/2: f' <= 0 everywhere, zero at q = 0 and q = 2), near-uniform density on a
+    jittered lattice, h from the unique-root bisection, momentum and energy identities."""
+    L = O.lib()
+    O.set_kernel(kernel)
+    try:
+        for q in np.linspace(0.0, 2.0, 41):
+            t = 1.0 - 0.5 * q
+            ref = {3: -5.0 * q * t ** 3, 4: -(7.0 / 3.0) * q * t ** 5 * (2.0 + 5.0 * q),
+                   5: -2.75 * q * t ** 7 * (2.0 + 7.0 * q + 8.0 * q * q)}[kernel]
+            assert L.orc_df(float(q)) == pytest.approx(ref, rel=1e-12, abs=1e-15)
+        w = W.cube(10, jitter=0.03, vel_amp=0.05, seed=4)
+        w.kernel = kernel
+        box, p = O.workload_box_params(w)
+        ev = O.evaluate(w.pos, w.vel, w.mass, w.u, w.h0, box, p, "brute")
+        # the self term over-estimates rho at ~58 neighbours, more for the more peaked functions (C2 < C4 < C6)
+        assert 0.0 < ev["rho"].mean() - 1.0 < (0.02, 0.03, 0.05)[kernel - 3] and ev["omega"].min() > 0.5
+        hb = O.h_bisect(w.pos, w.mass, box, p.hfact, 0.5 * ev["h"], 2.0 * ev["h"], kernel=kernel)
+        assert np.max(np.abs(hb / ev["h"] - 1)) < 1e-6
+        ma = (w.mass * ev["acc"]).sum(axis=1)
+        assert np.all(np.abs(ma) < 1e-13 * np.abs(w.mass * ev["acc"]).sum(axis=1).max())
+        de = (w.mass * ((w.vel * ev["acc"]).sum(axis=0) + ev["dudt"])).sum()
+        assert abs(de) < 1e-12 * (w.mass * np.abs(ev["dudt"])).sum()
+    finally:
+        O.set_kernel(0)
