@@ -69,7 +69,7 @@ typedef struct {
   int32_t max_h_iter;   /* 50  Newton iterations per particle per pass before SPH_ERR_H_NOCONV               */
   int32_t max_restarts; /* 50  chi-restarts per density solve before SPH_ERR_RESTARTS                        */
   int32_t eos;          /* 0 adiabatic; 1 locally isothermal c_s = cs0 (R/r0)^-q, du/dt = 0 (BASELINE cfg 3)  */
-  int32_t kernel;       /* 0 M4 (default; all BASELINE configs), 1 M5, 2 M6 (reading O6)            */
+  int32_t kernel;       /* 0 M4 (default; all BASELINE configs), 1 M5, 2 M6, 3/4/5 Wendland C2/C4/C6 (O6) */
   double cs0, r0, q;    /* locally isothermal EOS; R = cylindrical radius about centre[]                     */
   double GM, soft;      /* fixed point mass a_ext = -GM d / (|d|^2 + soft^2)^(3/2); GM = 0 disables          */
   double centre[3];

@@ -221,7 +221,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     c->N = N;
     c->box = *box;
     if (params) c->p = *params; else sph_default_params(&c->p);
-    if (c->p.kernel < 0 || c->p.kernel > 2) return fail(c, SPH_ERR_ARG, "kernel must be 0 (M4), 1 (M5) or 2 (M6)");
+    if (c->p.kernel < 0 || c->p.kernel >= kNumKernels) return fail(c, SPH_ERR_ARG, "kernel must be 0 (M4), 1 (M5), 2 (M6), 3 (Wendland C2), 4 (C4) or 5 (C6)");
     if (c->p.group_max == 0) c->p.group_max = kGroup;
     if (c->p.group_max < 1 || c->p.group_max > kGroup) return fail(c, SPH_ERR_ARG, "group_max must be in 1..32 (0 = default 32)");
     if (!(c->p.hfact > 0) || !(c->p.chi >= 1.0) || !(c->p.lambda > 1.0) || !(c->p.eps_h > 0) || c->p.max_h_iter < 1)

@@ -18,9 +18,14 @@ namespace sph {
 constexpr int kGroup = 32;          // leaf-group size bound: one warp lane per particle of a group
 // B-spline kernels (reading O6): 0 = M4 (cubic), 1 = M5 (quartic), 2 = M6 (quintic);
 // support radius in units of h and 3-D normalisation 1/pi, 1/(20 pi), 1/(120 pi)
-__host__ __device__ constexpr double kern_radius(int k) { return k == 0 ? 2.0 : (k == 1 ? 2.5 : 3.0); }
+// 3, 4, 5 = Wendland C2, C4, C6 on the support radius 2h: f = t^4 (1 + 2q), t^6 (1 + 3q + 35/12 q^2),
+// t^8 (1 + 4q + 25/4 q^2 + 4 q^3) with t = 1 - q/2; normalisations 21/(16 pi), 495/(256 pi), 1365/(512 pi)
+constexpr int kNumKernels = 6;
+__host__ __device__ constexpr double kern_radius(int k) { return k == 1 ? 2.5 : (k == 2 ? 3.0 : 2.0); }
 __host__ __device__ constexpr double kern_cnorm(int k) {
-    return k == 0 ? 0.31830988618379067154 : (k == 1 ? 0.31830988618379067154 / 20.0 : 0.31830988618379067154 / 120.0);
+    return k == 0 ? 0.31830988618379067154 : (k == 1 ? 0.31830988618379067154 / 20.0 : (k == 2 ? 0.31830988618379067154 / 120.0 :
+           (k == 3 ? 0.31830988618379067154 * 21.0 / 16.0 : (k == 4 ? 0.31830988618379067154 * 495.0 / 256.0 :
+                                                                      0.31830988618379067154 * 1365.0 / 512.0))));
 }
 
 // Sorted-order particle fields (SoA). Two sets are kept; the permute writes the other one.
@@ -231,6 +236,25 @@ __device__ __forceinline__ void kern_f_df(double q, double& f, double& df) {
         const double c1 = t1 * t1 * t1, c2 = t2 * t2 * t2, c3 = t3 * t3 * t3;
         f = fma(10.0 * c3, t3, fma(-5.0 * c2, t2, c1 * t1));
         df = -4.0 * fma(10.0, c3, fma(-5.0, c2, c1));
+    } else if (K >= 3) {
+        // Wendland: q is clamped to the support radius (integer compare of the high word, q >= +0), so that t = 0
+        // there and beyond and the polynomial factor cannot overflow for the density kernel's 1e100 padding entries;
+        // f' in factored form
+        const double qc = (__double2hiint(q) < 0x40000000) ? q : 2.0;
+        const double t = fma(-0.5, qc, 1.0), t2 = t * t;
+        if (K == 3) {
+            const double t3 = t2 * t;
+            f = t3 * t * fma(2.0, qc, 1.0);
+            df = -5.0 * qc * t3;
+        } else if (K == 4) {
+            const double t5 = t2 * t2 * t;
+            f = t5 * t * fma(qc, fma(35.0 / 12.0, qc, 3.0), 1.0);
+            df = (-7.0 / 3.0) * qc * t5 * fma(5.0, qc, 2.0);
+        } else {
+            const double t4 = t2 * t2, t7 = t4 * t2 * t;
+            f = t7 * t * fma(qc, fma(qc, fma(4.0, qc, 6.25), 4.0), 1.0);
+            df = -2.75 * qc * t7 * fma(qc, fma(8.0, qc, 7.0), 2.0);
+        }
     } else {
         const double a = 3.0 - q, b = 2.0 - q, c = 1.0 - q;
         const double t1 = clamp_pos(a), t2 = clamp_pos(b), t3 = clamp_pos(c);

@@ -269,7 +269,10 @@ static void density_launch(sph_ctx* c, size_t smem, const DensBox& db, const Den
                            uint32_t hi) {
     if (c->p.kernel == 0) density_launch_k<UNIM, GLOB, 0>(c, smem, db, dp, ncap, lo, hi);
     else if (c->p.kernel == 1) density_launch_k<UNIM, GLOB, 1>(c, smem, db, dp, ncap, lo, hi);
-    else density_launch_k<UNIM, GLOB, 2>(c, smem, db, dp, ncap, lo, hi);
+    else if (c->p.kernel == 2) density_launch_k<UNIM, GLOB, 2>(c, smem, db, dp, ncap, lo, hi);
+    else if (c->p.kernel == 3) density_launch_k<UNIM, GLOB, 3>(c, smem, db, dp, ncap, lo, hi);
+    else if (c->p.kernel == 4) density_launch_k<UNIM, GLOB, 4>(c, smem, db, dp, ncap, lo, hi);
+    else density_launch_k<UNIM, GLOB, 5>(c, smem, db, dp, ncap, lo, hi);
 }
 
 int launch_density(sph_ctx* c) {

@@ -291,8 +291,9 @@ def test_nonuniform_masses():
 
 @pytest.mark.parametrize("kernel,hfact,unequal,isothermal", [
     (0, 1.2, True, True), (1, 1.2, False, True), (1, 1.2, True, False), (1, 1.2, True, True),
-    (2, 1.0, False, True), (2, 1.0, True, False), (2, 1.0, True, True)],
-    ids=["M4_m_iso", "M5_iso", "M5_m", "M5_m_iso", "M6_iso", "M6_m", "M6_m_iso"])
+    (2, 1.0, False, True), (2, 1.0, True, False), (2, 1.0, True, True),
+    (3, 1.2, True, False), (4, 1.2, False, True), (5, 1.2, True, True)],
+    ids=["M4_m_iso", "M5_iso", "M5_m", "M5_m_iso", "M6_iso", "M6_m", "M6_m_iso", "C2_m", "C4_iso", "C6_m_iso"])
 def test_force_kernel_variants(kernel, hfact, unequal, isothermal):
     """The force kernel is compiled per (SPH kernel, equal masses or not, adiabatic or isothermal EOS): the staged
     rows differ (mass row dropped for equal masses, u row only for the adiabatic EOS; rho_b and P_b recomputed per
@@ -558,16 +559,18 @@ def test_corrector_recycle_parity():
     sim.close()
 
 
-@pytest.mark.parametrize("kernel,hfact", [(1, 1.2), (2, 1.0)], ids=["M5", "M6_hfact1"])
+@pytest.mark.parametrize("kernel,hfact", [(1, 1.2), (2, 1.0), (3, 1.2), (4, 1.2), (5, 1.3)],
+                         ids=["M5", "M6_hfact1", "WendlandC2", "WendlandC4", "WendlandC6_hfact1.3"])
 def test_other_kernels_stage_and_step_parity(kernel, hfact):
-    """M5 and M6 B-spline kernels (M6 with h_fact = 1.0 is the paper's physics-test setting,
-    PAPER.md:208): support radii 2.5 and 3 enter the traversal, the kernels the density and force loops."""
+    """M5 and M6 B-spline kernels and the Wendland functions C2, C4, C6 (M6 with h_fact = 1.0 is the
+    paper's physics-test setting): the support radii 2.5, 3 and 2 enter the traversal, the kernels the
+    density and force loops."""
     w = W.cube(14, jitter=0.08, vel_amp=0.03, seed=9)
     w.kernel, w.hfact = kernel, hfact
     w.h0 = np.full(w.n, hfact / 14)
     sim = _sim(w)
     ev, f = _stage_parity(w, sim)
-    assert ev["n_neigh"] / w.n > (100 if kernel == 1 else 130)
+    assert ev["n_neigh"] / w.n > {1: 100, 2: 130, 3: 70, 4: 70, 5: 85}[kernel]
     s = O.State(w, "grid")
     for _ in range(2):
         assert sim.step_leapfrog(want_dt=True) == pytest.approx(s.step(), rel=1e-9)
