@@ -111,10 +111,14 @@ def _f64(a):
 
 # ---- thin wrappers (marshalling only) ------------------------------------------------------------------------
 
-def morton_keys(pos, box: Box) -> np.ndarray:
+def morton_keys(pos, box: Box, beta: int = 21) -> np.ndarray:
+    """63-bit codes (beta = 21, the default) or the paper's shorter variant on a 2^beta grid (beta = 10: 30-bit codes)."""
     pos = _f64(pos)
     n = pos.shape[1]
     key = np.empty(n, dtype=np.uint64)
+    if beta != 21:
+        lib().orc_morton_keys_beta(C.c_int64(n), _p(pos, np.float64), C.byref(box), C.c_int32(int(beta)), _p(key, np.uint64))
+        return key
     lib().orc_morton_keys(C.c_int64(n), _p(pos, np.float64), C.byref(box), _p(key, np.uint64))
     return key
 

@@ -243,6 +243,33 @@ void orc_morton_keys(int64_t N, const double* pos, const orc_box* box, uint64_t*
     }
 }
 
+// The paper's 32-bit variant ("beta-bit" codes, 582 and 378: a 2^10 grid per axis, 30-bit codes): the same
+// definition on the 2^beta grid, 1 <= beta <= 21; the code occupies the low 3 beta bits (X0 at bit 3 beta - 1).
+void orc_morton_keys_beta(int64_t N, const double* pos, const orc_box* box, int32_t beta, uint64_t* key) {
+    double Lc = 0.0;
+    for (int c = 0; c < 3; ++c) Lc = std::max(Lc, box->hi[c] - box->lo[c]);
+    const double ng = (double)(1ull << beta);
+    for (int64_t i = 0; i < N; ++i) {
+        uint64_t X[3];
+        for (int c = 0; c < 3; ++c) {
+            double t = (pos[c * N + i] - box->lo[c]) / Lc;
+            uint64_t v = 0;
+            if (t > 0.0) {
+                double g = std::floor(t * ng);
+                v = (g >= ng - 1.0) ? (uint64_t)(ng - 1.0) : (uint64_t)g;
+            }
+            X[c] = v;
+        }
+        uint64_t m = 0;
+        for (int j = 0; j < beta; ++j)
+            for (int c = 0; c < 3; ++c) {
+                uint64_t bit = (X[c] >> (beta - 1 - j)) & 1u;
+                m |= bit << (3 * beta - 1 - 3 * j - c);
+            }
+        key[i] = m;
+    }
+}
+
 // worked example of PAPER.md:857-869 on beta-bit codes: delta, mask u << (beta - delta), prefix = a & mask.
 int32_t orc_delta_beta(uint64_t a, uint64_t b, int32_t beta) {
     uint64_t xr = a ^ b;

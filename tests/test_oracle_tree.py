@@ -182,3 +182,26 @@ def test_aabb_hmax_against_range_minmax():
         assert np.array_equal(box6[i, :3], ps[:, sl].min(axis=1))
         assert np.array_equal(box6[i, 3:], ps[:, sl].max(axis=1))
         assert hmax[i] == hs[sl].max()
+
+
+def test_morton_30bit_variant():
+    """The paper's 32-bit codes (2^10 cells per axis): grid coordinates floor(t 2^10), the same
+    interleave; since floor(floor(t 2^21) / 2^11) = floor(t 2^10), the 30-bit code is the top 30 bits of the 63-bit one."""
+    w = W.random_cloud(5000, seed=8)
+    box = O.make_box(w.box_lo, w.box_hi, w.periodic)
+    k30 = O.morton_keys(w.pos, box, beta=10)
+    assert np.all(k30 < 2 ** 30)
+    assert np.array_equal(k30, O.morton_keys(w.pos, box) >> np.uint64(33))
+    X = np.zeros((3, w.n), dtype=np.uint64)
+    for j in range(10):
+        for c in range(3):
+            X[c] |= ((k30 >> np.uint64(29 - 3 * j - c)) & np.uint64(1)) << np.uint64(9 - j)
+    assert np.array_equal(X, np.minimum(np.floor(w.pos * 1024.0), 1023).astype(np.uint64))
+    edge = np.array([[1.0, -0.5, 0.999999999], [7.0, 0.0, 0.5], [0.25, 0.25, 0.25]])
+    ke = O.morton_keys(edge, box, beta=10)
+    assert ke[0] >> np.uint64(29) == 1 and ke[1] < 2 ** 29          # clamp to the edge cells on both sides
+    # the tree over coarse codes has ties: broken by the sorted index, every internal node still splits its range
+    skey, perm = O.sort_keys(O.morton_keys(w.pos, box, beta=4))       # 4096 cells for 5000 particles
+    assert np.unique(skey).size < w.n
+    t = O.tree(skey)
+    assert np.all(t["rhi"] > t["rlo"])
