@@ -189,6 +189,7 @@ def main():
     ap.add_argument("--ref-side", type=int, default=40, help="lattice side of the oracle's bounded sample")
     ap.add_argument("--group-max", type=int, default=0,
                     help="particles per leaf group / bucket, 1..32 (0 = the default 32): the particles-per-leaf sweep of PAPER.md:382")
+    ap.add_argument("--morton-bits", type=int, default=0, help="21 (default) or 10: the paper's 30-bit Morton codes (PAPER.md:582, 378)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE config 4: sizes 64^3..512^3, one line each")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -216,7 +217,7 @@ def main():
 
     w = make_workload(args.workload, seed_offset=rank)
     n = w.n
-    sim = B.Sim.from_workload(w, params=B.params_for(w, group_max=args.group_max)) if args.group_max else B.Sim.from_workload(w)   # inputs resident in HBM; includes the white step
+    sim = B.Sim.from_workload(w, params=B.params_for(w, group_max=args.group_max, morton_bits=args.morton_bits))   # inputs resident in HBM; includes the white step
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -308,7 +309,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": "M4", "group_max": args.group_max or 32,
+                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": "M4", "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21,
                            "hfact": w.hfact, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "inputs (~0.8 kB/particle resident) larger than the 126 MB L2; no flush",
                            "restarts_last_step": st["restarts"], "h_iter_max": st["h_iter_max"]},

@@ -82,6 +82,11 @@ typedef struct {
   int32_t group_max;    /* 32   particles per leaf group / traversal bucket, 1..32 (0 = 32): the paper's particles-per-
                            leaf knob of the leaf reduction (Fig. 16). Results do
                            not depend on it (the neighbour sets are exact for any grouping); the speed does           */
+  int32_t morton_bits;  /* 21   grid bits per axis of the Morton code: 21 (63-bit codes) or 10, the paper's 32-bit variant
+                           (SURVEY.md 8(f) item 4): the 30-bit code is kept in the top bits of the
+                           64-bit key word (bits 62..33, the low 33 bits zero), sorted with four radix passes, ties
+                           (particles of one 2^-10 cell) stay in their previous order; results do not depend on it   */
+  int32_t reserved3;
 } sph_params;
 
 /* Device-memory hooks so that the host framework (PyTorch's caching allocator) owns device memory.

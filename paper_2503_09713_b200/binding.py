@@ -43,7 +43,7 @@ class Params(C.Structure):
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("kernel", C.c_int32), ("cs0", C.c_double),
                 ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
                 ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
-                ("max_recycle", C.c_int32), ("group_max", C.c_int32)]
+                ("max_recycle", C.c_int32), ("group_max", C.c_int32), ("morton_bits", C.c_int32), ("reserved3", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -127,6 +127,8 @@ def params_for(w, **kw) -> Params:
         extra.update(eps_v=w.eps_v)
     if getattr(w, "kernel", 0):
         extra.update(kernel=w.kernel)
+    if getattr(w, "morton_bits", 21) != 21:
+        extra.update(morton_bits=w.morton_bits)
     extra.update(kw)
     return default_params(**extra)
 

@@ -185,7 +185,7 @@ void sph_default_params(sph_params* p) {
     p->alpha_av = 1.0; p->beta_av = 2.0; p->beta_u = 1.0; p->c_cour = 0.3; p->c_force = 0.25;
     p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0; p->kernel = 0;
     p->cs0 = 1.0; p->r0 = 1.0; p->q = 0.0; p->GM = 0.0; p->soft = 0.0;
-    p->eps_v = 0.0; p->lambda_stiff = 2.0; p->max_recycle = 10; p->group_max = kGroup;
+    p->eps_v = 0.0; p->lambda_stiff = 2.0; p->max_recycle = 10; p->group_max = kGroup; p->morton_bits = 21;
 }
 
 const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
@@ -223,6 +223,8 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     if (params) c->p = *params; else sph_default_params(&c->p);
     if (c->p.kernel < 0 || c->p.kernel >= kNumKernels) return fail(c, SPH_ERR_ARG, "kernel must be 0 (M4), 1 (M5), 2 (M6), 3 (Wendland C2), 4 (C4) or 5 (C6)");
     if (c->p.group_max == 0) c->p.group_max = kGroup;
+    if (c->p.morton_bits == 0) c->p.morton_bits = 21;
+    if (c->p.morton_bits != 21 && c->p.morton_bits != 10) return fail(c, SPH_ERR_ARG, "morton_bits must be 21 or 10 (0 = default 21)");
     if (c->p.group_max < 1 || c->p.group_max > kGroup) return fail(c, SPH_ERR_ARG, "group_max must be in 1..32 (0 = default 32)");
     if (!(c->p.hfact > 0) || !(c->p.chi >= 1.0) || !(c->p.lambda > 1.0) || !(c->p.eps_h > 0) || c->p.max_h_iter < 1)
         return fail(c, SPH_ERR_ARG, "bad parameters");

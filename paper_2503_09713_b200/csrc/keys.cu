@@ -28,12 +28,13 @@ __device__ __forceinline__ uint64_t quantise(double x, double lo, double Lc) {
 
 __global__ void __launch_bounds__(256) k_morton(int64_t N, const double* __restrict__ x, const double* __restrict__ y,
                                                 const double* __restrict__ z, double lox, double loy, double loz,
-                                                double Lc, uint64_t* __restrict__ key, uint32_t* __restrict__ val) {
+                                                double Lc, uint64_t keep, uint64_t* __restrict__ key, uint32_t* __restrict__ val) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     uint64_t X = quantise(x[i], lox, Lc), Y = quantise(y[i], loy, Lc), Z = quantise(z[i], loz, Lc);
     // X0 Y0 Z0 X1 Y1 Z1 ... with X0 the most significant: X bit j -> key bit 3 j + 2
-    key[i] = (spread21(X) << 2) | (spread21(Y) << 1) | spread21(Z);
+    // keep = all ones, or the top 30 code bits only (morton_bits = 10: floor(t 2^10) = floor(t 2^21) >> 11 per axis)
+    key[i] = ((spread21(X) << 2) | (spread21(Y) << 1) | spread21(Z)) & keep;
     val[i] = (uint32_t)i;
 }
 
@@ -41,7 +42,8 @@ int launch_keys(sph_ctx* c) {
     double Lc = 0.0;
     for (int k = 0; k < 3; ++k) Lc = fmax(Lc, c->box.hi[k] - c->box.lo[k]);
     k_morton<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->box.lo[0], c->box.lo[1],
-                                                       c->box.lo[2], Lc, c->key, c->val);
+                                                       c->box.lo[2], Lc,
+                                                       c->p.morton_bits == 10 ? ~((1ull << 33) - 1ull) : ~0ull, c->key, c->val);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

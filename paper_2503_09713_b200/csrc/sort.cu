@@ -285,7 +285,9 @@ int launch_sort(sph_ctx* c) {
     unsigned hb = (unsigned)min((int64_t)148 * 8, (N + 255) / 256);
     // Prefix mode: sort on the top 40 bits only (five passes) and repair the rare runs of equal prefixes; chosen by
     // the host from the longest run seen in the previous sort (api.cu), all eight passes otherwise.
-    const int p0 = c->sort_p0;
+    // morton_bits = 10: the code sits in bits 62..33, four passes (bits 32..63) sort it completely, no repair
+    const bool short_codes = c->p.morton_bits == 10;
+    const int p0 = short_codes ? 4 : c->sort_p0;
     c->last_sort_passes = kPasses - p0;
     k_sort_hist<<<hb, 256, 0, c->stream>>>(c->key, N, c->sort_hist, p0);
     k_sort_bases<<<1, kRadix, 0, c->stream>>>(c->sort_hist, c->d_sc);
@@ -304,8 +306,10 @@ int launch_sort(sph_ctx* c) {
         std::swap(c->key, c->key_alt);
         std::swap(c->val, c->val_alt);
     }
-    k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, c->d_sc);
-    c->launches++;
+    if (!short_codes) {
+        k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, c->d_sc);
+        c->launches++;
+    }
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }

@@ -47,13 +47,17 @@ def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None):
     hn = w.h0 if hn is None else hn
     n = w.n
     # a1, a2: keys and permutation
-    skey, perm = O.sort_keys(O.morton_keys(pos, box))
+    beta = getattr(w, "morton_bits", 21)
+    skey, perm = O.sort_keys(O.morton_keys(pos, box, beta))
     gkey, gperm = sim.get_keys_perm()
+    if beta == 10:      # the 30-bit code is kept in bits 62..33 of the key word (include/sph_b200.h)
+        assert np.all(gkey & np.uint64((1 << 33) - 1) == 0)
+        gkey = gkey >> np.uint64(33)
     assert np.array_equal(gkey, skey), "sorted Morton keys differ"
     if np.unique(skey).size == n:
         assert np.array_equal(gperm, perm), "sort permutation differs"
     else:   # equal keys: ties follow the slot order at sort time, which is the original order only at step 0
-        assert np.array_equal(np.sort(gperm), np.arange(n)) and np.array_equal(O.morton_keys(pos, box)[gperm], skey)
+        assert np.array_equal(np.sort(gperm), np.arange(n)) and np.array_equal(O.morton_keys(pos, box, beta)[gperm], skey)
         if state is None:
             assert np.array_equal(gperm, perm)
     # a3: tree tables (Table B2 conventions)
@@ -659,3 +663,30 @@ def test_group_max_sweep_is_exact(gmax):
         sim.step_leapfrog(); sim.step_leapfrog()
         _invariants(w, sim)
         sim.close()
+
+
+@pytest.mark.parametrize("make", [
+    lambda: W.cube(16, jitter=0.05, vel_amp=0.02, seed=7),
+    lambda: W.random_cloud(5000, seed=3),
+    lambda: W.sod(16, 12),
+], ids=["cube16", "cloud_periodic", "sod_small"])
+def test_morton_30bit_variant_stage_and_step_parity(make):
+    """morton_bits = 10 (the paper's 32-bit codes): keys are the oracle's 30-bit codes, the sort
+    takes four passes, the tree over tied codes (a pair 1e-9 apart, four coincident particles) breaks ties on the
+    sorted index; every later stage is unchanged, and so is a two-step trajectory."""
+    w = make()
+    w.morton_bits = 10
+    w.pos[:, 200] = w.pos[:, 201] + 1e-9
+    w.pos[:, 100:104] = w.pos[:, 100:101]
+    sim = _sim(w)
+    _stage_parity(w, sim)
+    assert sim.stats()["sort_passes"] == 4
+    s = O.State(w, "grid")
+    for _ in range(2):
+        assert sim.step_leapfrog(want_dt=True) == pytest.approx(s.step(), rel=1e-9)
+    assert sim.stats()["sort_passes"] == 4
+    g = _np(sim.get_fields())
+    assert np.max(np.abs(g["pos"] - s.pos)) < 1e-12 and np.max(np.abs(g["h"] / s.h - 1)) < 1e-9
+    assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
+    _invariants(w, sim)
+    sim.close()
