@@ -36,7 +36,7 @@ FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
 # workload (profiles/r1_ncu_all_v22.md); only quoted when bench runs that workload
-NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.53e9, "traverse": 4.61e9, "density": 4.95e9}   # profiles/r1_ncu_all_v28.md
+NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.53e9, "traverse": 4.61e9, "density": 4.95e9}   # profiles/r1_ncu_all_v29.md
 
 
 def reduce_over_ranks(ms_local: float, n_local: float, world: int, device):
