@@ -36,6 +36,7 @@ FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
 # workload (profiles/r1_ncu_all_v22.md); only quoted when bench runs that workload
+KERNEL_NAMES = ("M4", "M5", "M6", "Wendland C2", "Wendland C4", "Wendland C6")   # FLOP_PER_PAIR_* below are the M4 counts
 NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.53e9, "traverse": 4.61e9, "density": 4.95e9}   # profiles/r1_ncu_all_v29.md
 
 
@@ -190,6 +191,8 @@ def main():
     ap.add_argument("--group-max", type=int, default=0,
                     help="particles per leaf group / bucket, 1..32 (0 = the default 32): the particles-per-leaf sweep of PAPER.md:382")
     ap.add_argument("--morton-bits", type=int, default=0, help="21 (default) or 10: the paper's 30-bit Morton codes (PAPER.md:582, 378)")
+    ap.add_argument("--sph-kernel", type=int, default=0, help="0 M4 (default, the BASELINE configs), 1 M5, 2 M6, 3/4/5 Wendland C2/C4/C6")
+    ap.add_argument("--hfact", type=float, default=0.0, help="h_fact (default 1.2; the paper uses 1.0 with M6, PAPER.md:208)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE config 4: sizes 64^3..512^3, one line each")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -216,6 +219,10 @@ def main():
             dist.barrier()
 
     w = make_workload(args.workload, seed_offset=rank)
+    if args.sph_kernel or args.hfact:      # other kernels: the same particles, h0 rescaled to the chosen h_fact
+        hf = args.hfact or w.hfact
+        w.h0 = w.h0 * (hf / w.hfact)
+        w.kernel, w.hfact = args.sph_kernel, hf
     n = w.n
     sim = B.Sim.from_workload(w, params=B.params_for(w, group_max=args.group_max, morton_bits=args.morton_bits))   # inputs resident in HBM; includes the white step
     stream = torch.cuda.current_stream()
@@ -297,7 +304,8 @@ def main():
                 kernels[k] = {"ms": v, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
         dom = max(per_stage, key=per_stage.get)
         roofline = dict(kernels[dom])
-        traffic = NCU_TRAFFIC_BYTES_CUBE256.get(dom) if args.workload == "cube256" else None
+        traffic = NCU_TRAFFIC_BYTES_CUBE256.get(dom) if (args.workload == "cube256" and not args.sph_kernel and not args.hfact
+                                                          and args.group_max in (0, 32)) else None
         roofline.update({"kernel": dom, "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
                          "peak_source": "sph_measure_fp64_peak DFMA microbenchmark, this run" if dom in flops else hbm_src,
                          "share_of_step": per_stage[dom] / sum(per_stage.values())})
@@ -309,7 +317,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": "M4", "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21,
+                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": KERNEL_NAMES[args.sph_kernel], "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21,
                            "hfact": w.hfact, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "inputs (~0.8 kB/particle resident) larger than the 126 MB L2; no flush",
                            "restarts_last_step": st["restarts"], "h_iter_max": st["h_iter_max"]},
