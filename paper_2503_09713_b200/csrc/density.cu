@@ -15,7 +15,9 @@
 namespace sph {
 
 constexpr int kDensWarps = 8;
-constexpr int kRegChunks = 12;    // 12 x 8 = 96 neighbours held in registers per octet
+constexpr int kRegChunks = 12;    // 12 x 8 = 96 neighbours held in registers per octet (kernels of radius 2)
+// M5 / M6 (radii 2.5 and 3: ~157 neighbours at h_fact 1.2 / 1.0) keep 20 x 8 = 160; their launches run 2 CTAs per SM
+template <int K> constexpr int kRegChunksK = (K == 1 || K == 2) ? 20 : kRegChunks;
 
 struct DensBox { double L[3], halfL[3]; int periodic[3]; };
 
@@ -87,14 +89,14 @@ struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
 template <bool WRAP, bool UNIM, bool GLOB, int K>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
                                             const uint32_t* __restrict__ cs,
-                                            const uint16_t* __restrict__ li, const uint32_t (&idx)[(kRegChunks + 1) / 2],
+                                            const uint16_t* __restrict__ li, const uint32_t (&idx)[(kRegChunksK<K> + 1) / 2],
                                             int n, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
-    double r[kRegChunks], mb[UNIM ? 1 : kRegChunks];
+    double r[kRegChunksK<K>], mb[UNIM ? 1 : kRegChunksK<K>];
     const double m0 = ma;                              // UNIM: every particle has this mass
 #pragma unroll
-    for (int c = 0; c < kRegChunks; ++c) {
+    for (int c = 0; c < kRegChunksK<K>; ++c) {
         const int k = c * 8 + (int)sl;
         r[c] = 1e100;                                  // q >> 2 (finite): outside the kernel support, contributes 0
         if (!UNIM) mb[c] = 0.0;
@@ -109,7 +111,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     auto sums = [&](double hinv, double& rho_sum, double& S) {
         double rs = 0.0, ss = 0.0;
 #pragma unroll
-        for (int c = 0; c < kRegChunks; ++c) {
+        for (int c = 0; c < kRegChunksK<K>; ++c) {
             double f, g;
             kern_f_g<K>(r[c] * hinv, f, g);
             if (UNIM) {
@@ -120,7 +122,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
                 ss = fma(mb[c], g, ss);
             }
         }
-        for (int k = kRegChunks * 8 + (int)sl; k < n; k += 8) {      // long lists: re-gather from smem
+        for (int k = kRegChunksK<K> * 8 + (int)sl; k < n; k += 8) {      // long lists: re-gather from smem
             uint32_t b = li[k];
             if (GLOB) b = cs[b];
             double f, g;
@@ -176,7 +178,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
 }
 
 template <bool UNIM, bool GLOB, int K>
-__global__ void __launch_bounds__(kDensWarps * 32, (UNIM && K == 0) ? 3 : 2) k_density(
+__global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) ? 3 : 2) k_density(
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
     const GroupRec* __restrict__ ginfo, const uint32_t* __restrict__ cslot, const uint32_t* __restrict__ cnt,
@@ -215,13 +217,13 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && K == 0) ? 3 : 2) k_d
     } else {
         sx = const_cast<double*>(x); sy = const_cast<double*>(y); sz = const_cast<double*>(z); sm = const_cast<double*>(m);
     }
-    // the first 96 list entries of the octet's particle (two 16-bit indices per register), in flight together with
+    // the first 96 (M5, M6: 160) list entries of the octet's particle (two 16-bit indices per register), in flight together with
     // the staging copies
-    uint32_t idx[(kRegChunks + 1) / 2];
+    uint32_t idx[(kRegChunksK<K> + 1) / 2];
 #pragma unroll
-    for (int c = 0; c < kRegChunks; c += 2) {
+    for (int c = 0; c < kRegChunksK<K>; c += 2) {
         const int k0 = c * 8 + (int)sl, k1 = k0 + 8;
-        const uint32_t i0 = (k0 < n) ? (uint32_t)li[k0] : 0u, i1 = (c + 1 < kRegChunks && k1 < n) ? (uint32_t)li[k1] : 0u;
+        const uint32_t i0 = (k0 < n) ? (uint32_t)li[k0] : 0u, i1 = (c + 1 < kRegChunksK<K> && k1 < n) ? (uint32_t)li[k1] : 0u;
         idx[c >> 1] = i0 | (i1 << 16);
     }
     cp_async_wait_all();

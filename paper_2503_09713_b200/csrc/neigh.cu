@@ -108,7 +108,7 @@ struct GroupCtx {
     uint32_t wpos;        // per lane, buffered mode: store position in the lane's row
     uint32_t nspill;      // per lane, buffered mode: hits of this group already spilled to the warp's global scratch
     bool hard_overflow;   // warp-uniform: a row could not spill any more (the group is walked a second time)
-    uint16_t* hspill;     // this lane's row of the warp's hit scratch
+    uint16_t* hspill;     // warp-uniform: the warp's hit scratch (row p = hspill + p * kSpillCap belongs to lane p)
     uint32_t ncs;         // warp-uniform: candidates (prefilter survivors) so far
     uint16_t* lptr;       // DIRECT: this lane's list in global memory
     uint32_t* cptr;       // candidate slots: the warp's scratch row, or (DIRECT) the group's array in global memory
@@ -234,7 +234,15 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             // when that is full too the group is counted on and walked a second time writing directly.
             if (__any_sync(0xffffffffu, G.wpos > (uint32_t)kHitCap)) {
                 if (!G.hard_overflow && __all_sync(0xffffffffu, G.nspill + G.wpos <= (uint32_t)kSpillCap)) {
-                    for (uint32_t k = 0; k < G.wpos; ++k) G.hspill[G.nspill + k] = s.hits[row + k];
+                    // the warp moves one row at a time (coalesced 16-bit stores; lane by lane the stores of a row
+                    // fell into 32 different sectors per instruction)
+                    __syncwarp();
+                    for (uint32_t p = 0; p < 32u; ++p) {
+                        const uint32_t wn = __shfl_sync(0xffffffffu, G.wpos, p), ns = __shfl_sync(0xffffffffu, G.nspill, p);
+                        uint16_t* dst = G.hspill + (size_t)p * kSpillCap + ns;
+                        for (uint32_t k = lane; k < wn; k += 32) dst[k] = s.hits[p * kHitStride + k];
+                    }
+                    __syncwarp();
                     G.nspill += G.wpos;
                     G.wpos = 0u;
                 } else {
@@ -474,7 +482,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         }
         if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
-        G.hspill = hit_row + (size_t)lane * kSpillCap;
+        G.hspill = hit_row;
 
         if (nu >= 0) refine<false>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
         else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
