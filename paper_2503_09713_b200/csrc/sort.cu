@@ -16,8 +16,9 @@ constexpr int kPrefixPass = 3;                   // prefix mode sorts on digits 
 constexpr int kPrefixShift = kPrefixPass * 8;
 constexpr int kSortThreads = 512;
 constexpr int kSortWarps = kSortThreads / 32;
-constexpr int kItems = 8;                        // keys per thread
-constexpr int kTile = kSortThreads * kItems;     // 4096 keys per tile
+constexpr int kItems = 10;                       // keys per thread
+constexpr int kTile = kSortThreads * kItems;     // 5120 keys per tile, 2 CTAs = 32 warps per SM (8 keys per thread at 3 CTAs
+                                                 // per SM: 0.99 instead of 0.93 ms at C2; 12 keys spill at 64 registers)
 constexpr int kLookBatch = 4;
 __device__ __forceinline__ uint32_t pad(uint32_t j) { return j + (j >> 5); }
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
@@ -103,7 +104,7 @@ struct SortSmem {
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(kSortThreads, 3) k_onesweep(const uint64_t* __restrict__ kin,
+__global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint64_t* __restrict__ kin,
                                                             const uint32_t* __restrict__ vin,
                                                             uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                             int64_t N, int shift, const uint32_t* __restrict__ gbase,
