@@ -13,7 +13,9 @@
 // itself -- worked examples printed in the paper (delta/prefix example PAPER.md:833-869, Table B2
 // PAPER.md:899-907), brute force, closed forms (int W dV = 1, W(0) = 1/(pi h^3)), the unique-root bisection
 // for h, conservation identities (sum m a = 0, sum m (v.a + du/dt) = 0), Galilean invariance, the exact
-// Riemann solution for the Sod tube. "parity unpinned": none.
+// Riemann solution for the Sod tube; the magnitudes the identities cannot see -- the 1/2 and v_sig of Eq. 5-6, the
+// 1/2, beta_u and mean density of Eq. 8-9, F_ab(h_a) against F_ab(h_b), the force term and the pair maximum of G8 --
+// by five two-particle cases worked by hand (tests/golden/pair_forces.txt). "parity unpinned": none.
 //
 // Layout convention: vectors are SoA, pos = x[0..N) y[0..N) z[0..N) contiguous (3N doubles).
 
