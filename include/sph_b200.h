@@ -124,6 +124,8 @@ typedef struct {
   int32_t recycles;        /* corrector re-cycles of the last step (eps_v > 0)                              */
   int32_t reserved;
   double cfl_mult;         /* CFL multiplier lambda_CFL applied to the next internal dt                     */
+  int64_t density_sweeps;  /* sweeps over the neighbour lists executed by the last density pass, summed over
+                              particles: Newton sweeps + the closing pass at the converged h (Omega)         */
 } sph_stats;
 
 void sph_default_params(sph_params* p);
@@ -137,7 +139,12 @@ int sph_init(sph_ctx** out, int64_t N, const double* pos_dev, const double* vel_
 
 /* sph_init_ex: same with everything explicit. mem says where pos/vel/mass/u/h0 live. h0 (N) may be NULL.
  * params NULL = defaults. cuda_stream is a cudaStream_t (NULL = default stream). allocator may be NULL.
- * If run_white_step is 0 the caller drives sph_build_tree / sph_compute_density / sph_compute_forces. */
+ * If run_white_step is 0 the caller drives sph_build_tree / sph_compute_density / sph_compute_forces.
+ * The context lives on the CUDA device that is current at this call; every later call makes that device current
+ * for its duration, so contexts on several devices may coexist in one process.
+ * On failure: if the arguments themselves are invalid or no sm_100 device is present, *out is NULL; for any later
+ * failure (allocation, a parameter out of range, an error of the white step) *out is a live context whose only
+ * valid uses are sph_last_error() and sph_free(): the caller must free it. */
 int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const double* vel, const double* mass,
                 const double* u, const double* h0, const sph_box* box, const sph_params* params,
                 void* cuda_stream, const sph_allocator* allocator, int run_white_step);
@@ -186,6 +193,12 @@ int sph_get_tree(sph_ctx* ctx, sph_mem mem, int32_t* left, int32_t* right, uint8
 /* Neighbour cache as CSR over sorted slots: offs[N+1], idx[cap] (sorted-slot indices, unordered within a list).
  * idx may be NULL to query offs only; SPH_ERR_CAP if cap < offs[N]. */
 int sph_get_neighbours(sph_ctx* ctx, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap);
+/* The same for the sorted slots [first, first + count) only (parity checks on samples of a large run, where the whole
+ * CSR would be several GB): offs[count + 1] are the ABSOLUTE offsets offs_all[first .. first + count], idx[cap]
+ * receives the lists of those slots back to back (list of slot first + k at idx[offs[k] - offs[0]]).
+ * SPH_ERR_ARG if the range leaves [0, N); SPH_ERR_CAP if cap < offs[count] - offs[0]. */
+int sph_get_neighbours_range(sph_ctx* ctx, sph_mem mem, int64_t first, int64_t count, uint64_t* offs, uint32_t* idx,
+                             uint64_t cap);
 int sph_get_stats(sph_ctx* ctx, sph_stats* out);
 int sph_reset_timers(sph_ctx* ctx);
 const char* sph_last_error(const sph_ctx* ctx);

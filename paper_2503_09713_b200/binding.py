@@ -22,7 +22,7 @@ STATUS = {0: "SPH_OK", -1: "SPH_ERR_ARG", -2: "SPH_ERR_DEVICE", -3: "SPH_ERR_OOM
 # every symbol include/sph_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["sph_default_params", "sph_init", "sph_init_ex", "sph_build_tree", "sph_compute_density",
            "sph_compute_forces", "sph_step_leapfrog", "sph_set_fields", "sph_get_fields", "sph_get_keys_perm",
-           "sph_get_tree", "sph_get_neighbours", "sph_get_stats", "sph_reset_timers", "sph_last_error", "sph_free",
+           "sph_get_tree", "sph_get_neighbours", "sph_get_neighbours_range", "sph_get_stats", "sph_reset_timers", "sph_last_error", "sph_free",
            "sph_measure_fp64_peak"]
 
 
@@ -62,7 +62,8 @@ class Stats(C.Structure):
                 ("restarts", C.c_int32), ("steps", C.c_int64), ("kernel_launches", C.c_int64), ("dt", C.c_double),
                 ("t", C.c_double), ("bytes_allocated", C.c_int64), ("cand_max", C.c_int32), ("groups_fallback", C.c_int32),
                 ("chunks_shared", C.c_int32), ("share_chunk", C.c_int32), ("sort_passes", C.c_int32),
-                ("sort_tie_max", C.c_int32), ("recycles", C.c_int32), ("reserved", C.c_int32), ("cfl_mult", C.c_double)]
+                ("sort_tie_max", C.c_int32), ("recycles", C.c_int32), ("reserved", C.c_int32), ("cfl_mult", C.c_double),
+                ("density_sweeps", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -94,6 +95,7 @@ def load():
         lib.sph_get_keys_perm.argtypes = [vp, C.c_int, vp, vp]
         lib.sph_get_tree.argtypes = [vp, C.c_int] + [vp] * 9
         lib.sph_get_neighbours.argtypes = [vp, C.c_int, vp, vp, C.c_uint64]
+        lib.sph_get_neighbours_range.argtypes = [vp, C.c_int, i64, i64, vp, vp, C.c_uint64]
         lib.sph_get_stats.argtypes = [vp, C.POINTER(Stats)]
         lib.sph_measure_fp64_peak.argtypes = [C.POINTER(dbl), vp]
         _lib = lib
@@ -195,6 +197,27 @@ class Sim:
         self._check(rc)
 
     @classmethod
+    def from_sph_init(cls, pos, vel, mass, u, box_lo, box_hi, periodic, gamma: float, hfact: float):
+        """north_star's entry point ``sph_init``: device tensors, default parameters with the given gamma and hfact,
+        the NULL stream, cudaMalloc, no initial smoothing lengths (fallback of reading A9); runs the white step."""
+        import torch
+        self = cls.__new__(cls)
+        self.torch, self.lib = torch, load()
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        self.stream = torch.cuda.default_stream()
+        self.n = int(pos.shape[1])
+        self.box = Box((C.c_double * 3)(*box_lo), (C.c_double * 3)(*box_hi), (C.c_int32 * 3)(*[int(x) for x in periodic]))
+        self.params = default_params(gamma=gamma, hfact=hfact)
+        self._allocator = None
+        args = [a.contiguous() for a in (pos, vel, mass, u)]
+        assert all(a.is_cuda and a.dtype == torch.float64 for a in args)
+        torch.cuda.synchronize()          # the inputs were produced on torch's stream; sph_init works on the NULL stream
+        self.ctx = C.c_void_p()
+        self._check(self.lib.sph_init(C.byref(self.ctx), self.n, *[_ptr(a) for a in args], C.byref(self.box),
+                                      float(gamma), float(hfact)))
+        return self
+
+    @classmethod
     def from_workload(cls, w, device_inputs: bool = True, **kw):
         import torch
         params = kw.pop("params", None) or params_for(w)
@@ -293,6 +316,14 @@ class Sim:
         idx = np.empty(int(offs[-1]), dtype=np.uint32)
         self._check(self.lib.sph_get_neighbours(self.ctx, SPH_MEM_HOST, _ptr(offs), _ptr(idx), idx.size))
         return offs, idx
+
+    def get_neighbours_range(self, first: int, count: int):
+        """Lists of the sorted slots [first, first + count): (offs relative to the first list, idx)."""
+        offs = np.empty(count + 1, dtype=np.uint64)
+        self._check(self.lib.sph_get_neighbours_range(self.ctx, SPH_MEM_HOST, first, count, _ptr(offs), None, 0))
+        idx = np.empty(int(offs[-1] - offs[0]), dtype=np.uint32)
+        self._check(self.lib.sph_get_neighbours_range(self.ctx, SPH_MEM_HOST, first, count, _ptr(offs), _ptr(idx), idx.size))
+        return offs - offs[0], idx
 
     def stats(self) -> dict:
         s = Stats()

@@ -37,15 +37,15 @@ static int dalloc(sph_ctx* c, T** out, size_t count) {
     size_t bytes = std::max<size_t>(count * sizeof(T), 256);
     void* p = c->alloc.alloc(bytes, c->alloc.user);
     if (!p) return fail(c, SPH_ERR_OOM, "device allocation of %zu bytes failed", bytes);
-    c->allocations.push_back(p);
+    c->allocations.emplace_back(p, bytes);
     c->bytes_allocated += (int64_t)bytes;
     *out = reinterpret_cast<T*>(p);
     return SPH_OK;
 }
 static void dfree(sph_ctx* c, void* p) {
     if (!p) return;
-    auto it = std::find(c->allocations.begin(), c->allocations.end(), p);
-    if (it != c->allocations.end()) c->allocations.erase(it);
+    auto it = std::find_if(c->allocations.begin(), c->allocations.end(), [p](const std::pair<void*, size_t>& a) { return a.first == p; });
+    if (it != c->allocations.end()) { c->bytes_allocated -= (int64_t)it->second; c->allocations.erase(it); }
     c->alloc.release(p, c->alloc.user);
 }
 
@@ -83,11 +83,35 @@ struct StageTimer {
     }
 };
 
+// after a stream synchronisation every recorded stage timer is complete: add it to the per-stage totals and hand its
+// events back to the pool (a long run keeps a bounded number of events)
+static void fold_timers(sph_ctx* c) {
+    for (auto& t : c->timers) {
+        float v = 0.f;
+        if (cudaEventElapsedTime(&v, t.e0, t.e1) == cudaSuccess) c->ms_acc[t.stage] += v; else cudaGetLastError();
+        c->event_pool.push_back(t.e0);
+        c->event_pool.push_back(t.e1);
+    }
+    c->timers.clear();
+}
+
 static int read_scalars(sph_ctx* c) {
     SPH_CUDA(c, cudaMemcpyAsync(c->h_sc, c->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    fold_timers(c);
     return SPH_OK;
 }
+
+// Every ABI entry makes the context's device current for its duration (function attributes, launches and events are
+// per device) and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const sph_ctx* c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 __global__ void k_iota(int64_t N, uint32_t* id) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -101,12 +125,25 @@ __global__ void k_fill(int64_t N, double* p, double v) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) p[i] = v;
 }
-// fallback h0 = hfact (m V / M_tot)^(1/3) (reading A9); M_tot by a simple two-kernel reduction
-__global__ void k_sum(int64_t N, const double* __restrict__ m, double* out) {
+// fallback h0 = hfact (m V / M_tot)^(1/3) (reading A9); M_tot by a two-stage reduction in a fixed order (per-block
+// partials over a fixed grid, then one block), so that the initial h is reproducible bit for bit
+__global__ void __launch_bounds__(256) k_sum_partial(int64_t N, const double* __restrict__ m, double* __restrict__ part) {
+    __shared__ double ws[8];
     double v = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) v += m[i];
     v = warp_sum(v);
-    if (lane_id() == 0) atomicAdd(out, v);
+    if (lane_id() == 0) ws[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = ws[0];
+        for (int w = 1; w < 8; ++w) t += ws[w];
+        part[blockIdx.x] = t;
+    }
+}
+__global__ void k_sum_final(int nblocks, const double* __restrict__ part, double* out) {
+    double t = 0.0;
+    for (int b = 0; b < nblocks; ++b) t += part[b];
+    *out = t;
 }
 __global__ void k_h0_fallback(int64_t N, const double* __restrict__ m, const double* mtot, double vol, double hfact, double* h) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -127,12 +164,15 @@ static int grow_pool(sph_ctx* c, T** pool, uint64_t* cap, uint64_t want) {
 // neighbour cache for the current tree and h^n: hmax -> AABB -> single traversal pass (count, allocate, fill per
 // group from bump allocators). The pass is repeated with larger pools if one of them overflowed (first build,
 // or a cache that grew by more than the slack since the previous step).
+constexpr int kSortRedo = 1;   // cache_build: the prefix-mode sort gave up on a long run; sort again in full
+
 static int cache_build(sph_ctx* c) {
     { StageTimer t(c, ST_AABB); SPH_TRY(launch_hmax(c)); SPH_TRY(launch_aabb(c)); }
     for (int attempt = 0;; ++attempt) {
         { StageTimer t(c, ST_TRAVERSE); SPH_TRY(launch_traverse(c)); }
         SPH_TRY(read_scalars(c));
         const DevScalars& s = *c->h_sc;
+        if (s.sort_redo) { c->sort_p0 = 0; return kSortRedo; }
         for (int k = 0; k < 3; ++k)
             if (c->box.periodic[k] && !(2.0 * kern_radius(c->p.kernel) * c->p.chi * s.h_max < c->box.hi[k] - c->box.lo[k]))
                 return fail(c, SPH_ERR_PERIODIC_TOO_SMALL, "periodic axis %d: 2 R_kern chi h_max = %g >= L = %g", k,
@@ -192,11 +232,12 @@ const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context
 
 void sph_free(sph_ctx* c) {
     if (!c) return;
+    DeviceGuard dg(c);
     cudaStreamSynchronize(c->stream);
     for (auto& t : c->timers) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
     for (auto e : c->event_pool) cudaEventDestroy(e);
-    std::vector<void*> all = c->allocations;
-    for (void* p : all) c->alloc.release(p, c->alloc.user);
+    for (auto& a : c->allocations) c->alloc.release(a.first, c->alloc.user);
+    c->allocations.clear();
     if (c->h_sc) cudaFreeHost(c->h_sc);
     delete c;
 }
@@ -219,6 +260,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     if (!c) return SPH_ERR_OOM;
     *out = c;   // returned even on failure so that sph_last_error() can be read; caller frees it
     c->N = N;
+    c->device = dev;
     c->box = *box;
     if (params) c->p = *params; else sph_default_params(&c->p);
     if (c->p.kernel < 0 || c->p.kernel >= kNumKernels) return fail(c, SPH_ERR_ARG, "kernel must be 0 (M4), 1 (M5), 2 (M6), 3 (Wendland C2), 4 (C4) or 5 (C6)");
@@ -281,9 +323,11 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
         double vol = 1.0;
         for (int k = 0; k < 3; ++k) vol *= box->hi[k] - box->lo[k];
         double* mtot = c->d_dtstep + 1;
-        k_sum<<<(unsigned)std::min<int64_t>(592, (N + 255) / 256), 256, 0, c->stream>>>(N, c->cur.m, mtot);
+        const unsigned nb = (unsigned)std::min<int64_t>(592, (N + 255) / 256);   // corr_part holds >= 2 ceil(N / 256) doubles
+        k_sum_partial<<<nb, 256, 0, c->stream>>>(N, c->cur.m, c->corr_part);
+        k_sum_final<<<1, 1, 0, c->stream>>>((int)nb, c->corr_part, mtot);
         k_h0_fallback<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, mtot, vol, c->p.hfact, c->cur.h);
-        c->launches += 2;
+        c->launches += 3;
     }
     k_mass_uniform<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, c->d_sc);
     c->launches++;
@@ -310,17 +354,25 @@ int sph_init(sph_ctx** out, int64_t N, const double* pos_dev, const double* vel_
 
 int sph_build_tree(sph_ctx* c) {
     SPH_TRY(check_ctx(c));
-    { StageTimer t(c, ST_KEYS); SPH_TRY(launch_keys(c)); }
-    { StageTimer t(c, ST_SORT); SPH_TRY(launch_sort(c)); }
-    { StageTimer t(c, ST_PERMUTE); SPH_TRY(launch_permute(c)); }
-    { StageTimer t(c, ST_TREE); SPH_TRY(launch_tree(c)); }
-    SPH_TRY(cache_build(c));
+    DeviceGuard dg(c);
+    for (int attempt = 0;; ++attempt) {
+        { StageTimer t(c, ST_KEYS); SPH_TRY(launch_keys(c)); }
+        { StageTimer t(c, ST_SORT); SPH_TRY(launch_sort(c)); }
+        { StageTimer t(c, ST_PERMUTE); SPH_TRY(launch_permute(c)); }
+        { StageTimer t(c, ST_TREE); SPH_TRY(launch_tree(c)); }
+        const int rc = cache_build(c);
+        if (rc == SPH_OK) break;
+        // the prefix-mode sort met a run too long to repair (the tree kernels then did nothing): the fields are a
+        // valid permutation of the particles, so the build simply starts over with all eight radix passes
+        if (rc != kSortRedo || attempt > 0) return rc == kSortRedo ? fail(c, SPH_ERR_DEVICE, "sort did not complete") : rc;
+    }
     c->state = S_TREE;
     return SPH_OK;
 }
 
 int sph_compute_density(sph_ctx* c) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "sph_compute_density needs sph_build_tree first");
     int restarts = 0;
     for (;;) {
@@ -351,6 +403,7 @@ static int forces_eval(sph_ctx* c) {
 
 int sph_compute_forces(sph_ctx* c) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     SPH_TRY(forces_eval(c));
     // standalone evaluation (and the white step): the result becomes a^n, du/dt^n of the next predictor
     StageTimer t(c, ST_LEAPFROG);
@@ -359,6 +412,7 @@ int sph_compute_forces(sph_ctx* c) {
 
 int sph_step_leapfrog(sph_ctx* c, double dt, double* dt_used) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (!c->have_cfl_dt) return fail(c, SPH_ERR_ORDER, "sph_step_leapfrog needs a force evaluation (a^n, dt) first");
     {
         StageTimer t(c, ST_LEAPFROG);
@@ -422,6 +476,7 @@ static int copy_out(sph_ctx* c, sph_mem mem, const double* src_sorted, double* d
 int sph_set_fields(sph_ctx* c, sph_mem mem, const double* pos, const double* vel, const double* u, const double* h,
                    const double* acc, const double* dudt) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     double* stage = nullptr;   // one staging buffer reused in stream order
     int rc = SPH_OK;
     if ((rc = copy_in(c, mem, pos, c->cur.x, 3, &stage)) == SPH_OK && (rc = copy_in(c, mem, vel, c->cur.vx, 3, &stage)) == SPH_OK &&
@@ -431,12 +486,14 @@ int sph_set_fields(sph_ctx* c, sph_mem mem, const double* pos, const double* vel
     if (stage) { cudaStreamSynchronize(c->stream); dfree(c, stage); }
     if (rc != SPH_OK) return rc;
     if (pos || vel || u || h) c->state = S_FIELDS;
+    if (pos) c->sort_p0 = 0;   // unrelated positions: the previous order says nothing about the next sort's ties
     return SPH_OK;
 }
 
 int sph_get_fields(sph_ctx* c, sph_mem mem, double* pos, double* vel, double* u, double* h, double* rho, double* omega,
                    double* acc, double* dudt) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if ((rho || omega) && c->state < S_DENSITY) return fail(c, SPH_ERR_ORDER, "rho/omega need sph_compute_density");
     double* stage = nullptr;
     int rc = SPH_OK;
@@ -463,6 +520,7 @@ static int copy_raw(sph_ctx* c, sph_mem mem, void* dst, const void* src_dev, siz
 
 int sph_get_keys_perm(sph_ctx* c, sph_mem mem, uint64_t* sorted_keys, uint32_t* perm) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no tree built");
     SPH_TRY(copy_raw(c, mem, sorted_keys, c->key, (size_t)c->N * sizeof(uint64_t)));
     SPH_TRY(copy_raw(c, mem, perm, c->cur.id, (size_t)c->N * sizeof(uint32_t)));
@@ -489,6 +547,7 @@ __global__ void k_export_tree(int64_t N, const NodeRec* __restrict__ nodes, int3
 int sph_get_tree(sph_ctx* c, sph_mem mem, int32_t* left, int32_t* right, uint8_t* lflag, uint8_t* rflag, int32_t* parent,
                  int32_t* range_lo, int32_t* range_hi, double* aabb, double* hmax) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no tree built");
     const int64_t N = c->N, ni = N - 1;
     if (parent) {
@@ -515,20 +574,27 @@ int sph_get_tree(sph_ctx* c, sph_mem mem, int32_t* left, int32_t* right, uint8_t
     return rc;
 }
 
-int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
+int sph_get_neighbours_range(sph_ctx* c, sph_mem mem, int64_t first, int64_t count, uint64_t* offs, uint32_t* idx, uint64_t cap) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no neighbour cache built");
-    // the cache is group-local (bucket tables + 16-bit lists); convert to a CSR over sorted slots on request
+    if (first < 0 || count < 1 || first + count > c->N) return fail(c, SPH_ERR_ARG, "slot range [%lld, %lld) outside [0, N)", (long long)first, (long long)(first + count));
+    // the cache is group-local (candidate arrays + 16-bit lists); convert to a CSR over sorted slots on request
     SPH_TRY(launch_scan_u32_u64(c, c->cnt, c->offs, c->N, nullptr));
-    SPH_TRY(copy_raw(c, mem, offs, c->offs, (size_t)(c->N + 1) * sizeof(uint64_t)));
+    uint64_t ends[2] = {0, 0};
+    SPH_CUDA(c, cudaMemcpyAsync(&ends[0], c->offs + first, sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaMemcpyAsync(&ends[1], c->offs + first + count, sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
+    SPH_TRY(copy_raw(c, mem, offs, c->offs + first, (size_t)(count + 1) * sizeof(uint64_t)));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     if (idx) {
-        if (cap < c->n_neigh) return fail(c, SPH_ERR_CAP, "idx capacity %llu < %llu neighbours", (unsigned long long)cap,
-                                          (unsigned long long)c->n_neigh);
+        const uint64_t total = ends[1] - ends[0];
+        if (cap < total) return fail(c, SPH_ERR_CAP, "idx capacity %llu < %llu neighbours", (unsigned long long)cap,
+                                     (unsigned long long)total);
         uint32_t* tmp = nullptr;
         uint32_t* dst = idx;
-        if (mem == SPH_MEM_HOST) { SPH_TRY(dalloc(c, &tmp, (size_t)c->n_neigh + 1)); dst = tmp; }
-        int rc = launch_cache_to_csr(c, dst);
-        if (rc == SPH_OK && tmp) rc = copy_raw(c, mem, idx, tmp, (size_t)c->n_neigh * sizeof(uint32_t));
+        if (mem == SPH_MEM_HOST) { SPH_TRY(dalloc(c, &tmp, (size_t)total + 1)); dst = tmp; }
+        int rc = launch_cache_to_csr(c, dst, first, count);
+        if (rc == SPH_OK && tmp) rc = copy_raw(c, mem, idx, tmp, (size_t)total * sizeof(uint32_t));
         cudaStreamSynchronize(c->stream);
         if (tmp) dfree(c, tmp);
         if (rc != SPH_OK) return rc;
@@ -537,25 +603,28 @@ int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, u
     return SPH_OK;
 }
 
+int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
+    SPH_TRY(check_ctx(c));
+    return sph_get_neighbours_range(c, mem, 0, c->N, offs, idx, cap);
+}
+
 int sph_reset_timers(sph_ctx* c) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
-    for (auto& t : c->timers) { c->event_pool.push_back(t.e0); c->event_pool.push_back(t.e1); }
-    c->timers.clear();
+    fold_timers(c);
+    for (int k = 0; k < ST_COUNT; ++k) c->ms_acc[k] = 0.0;
     c->launches = 0;
     return SPH_OK;
 }
 
 int sph_get_stats(sph_ctx* c, sph_stats* out) {
     SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
     if (!out) return SPH_ERR_ARG;
     memset(out, 0, sizeof(*out));
     SPH_TRY(read_scalars(c));
-    double ms[ST_COUNT] = {0};
-    for (auto& t : c->timers) {
-        float v = 0.f;
-        if (cudaEventElapsedTime(&v, t.e0, t.e1) == cudaSuccess) ms[t.stage] += v; else cudaGetLastError();
-    }
+    const double* ms = c->ms_acc;               // read_scalars synchronised and folded every open timer
     out->ms_keys = ms[ST_KEYS]; out->ms_sort = ms[ST_SORT]; out->ms_permute = ms[ST_PERMUTE]; out->ms_tree = ms[ST_TREE];
     out->ms_aabb = ms[ST_AABB]; out->ms_traverse = ms[ST_TRAVERSE]; out->ms_scan = ms[ST_SCAN];
     out->ms_density = ms[ST_DENSITY]; out->ms_forces = ms[ST_FORCES]; out->ms_leapfrog = ms[ST_LEAPFROG];
@@ -569,7 +638,7 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
     out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
     out->sort_passes = c->last_sort_passes; out->sort_tie_max = (int32_t)s.tie_max;
-    out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult;
+    out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult; out->density_sweeps = (int64_t)s.sweeps;
     return SPH_OK;
 }
 

@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <utility>
 #include <vector>
 
 #include "../../include/sph_b200.h"
@@ -78,6 +79,10 @@ struct DevScalars {
     unsigned int tie_max;            // longest run of keys equal in their top 40 bits (sort prefix mode)
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
+    unsigned int sort_redo;          // prefix-mode sort met a run of equal prefixes too long to repair: the tree kernels
+                                     // of this build do nothing and the host sorts again with all eight passes
+    unsigned long long sweeps;       // Newton sweeps + closing passes executed by the last density launch, summed over
+                                     // particles (bench.py: measured flop count of k_density)
 };
 
 struct TimerRec { int stage; cudaEvent_t e0, e1; };
@@ -90,8 +95,9 @@ struct sph_ctx {
     sph_params p{};
     cudaStream_t stream = nullptr;
     sph_allocator alloc{};
+    int device = 0;                     // the CUDA device this context lives on (every ABI entry makes it current)
     int64_t bytes_allocated = 0;
-    std::vector<void*> allocations;
+    std::vector<std::pair<void*, size_t>> allocations;
 
     sph::Fields cur{}, alt{};
     double *rho = nullptr, *omega = nullptr, *P = nullptr, *cs = nullptr, *A = nullptr;   // A = 1/(rho^2 Omega)
@@ -152,8 +158,9 @@ struct sph_ctx {
     uint32_t last_chunk = 1;
     bool uniform_mass = false;          // all particle masses equal (density kernel variant)
 
-    std::vector<sph::TimerRec> timers;
+    std::vector<sph::TimerRec> timers;  // open since the last stream synchronisation; folded into ms_acc there
     std::vector<cudaEvent_t> event_pool;
+    double ms_acc[sph::ST_COUNT] = {0};
     char err[512] = {0};
 };
 
@@ -183,9 +190,9 @@ int launch_permute(sph_ctx* c);                                // permute.cu
 int launch_tree(sph_ctx* c);                                   // tree.cu   karras + groups
 int launch_aabb(sph_ctx* c);                                   // tree.cu
 int launch_traverse(sph_ctx* c);                               // neigh.cu  single pass: walk, test, write cache
-int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out);
+int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out, int64_t first, int64_t count);   // neigh.cu  group-local lists -> CSR (getter)
 size_t trav_hit_scratch_entries();                              // neigh.cu  u16 entries of the traversal's hit spill rows
-size_t trav_scratch_entries();                                  // neigh.cu  u32 entries of the traversal's scratch rows        // neigh.cu  group-local lists -> global CSR (getter)
+size_t trav_scratch_entries();                                  // neigh.cu  u32 entries of the traversal's scratch rows
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
 int launch_density(sph_ctx* c);                                // density.cu

@@ -243,38 +243,41 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) 
     unsigned itm = (unsigned)o.it;
 #pragma unroll
     for (int ofs = 16; ofs > 0; ofs >>= 1) itm = max(itm, __shfl_xor_sync(0xffffffffu, itm, ofs));
+    // executed sweeps of this warp's particles: Newton sweeps + the closing pass at the final h (bench.py's flop count)
+    unsigned swp = (pv && sl == 0u) ? (unsigned)o.it + 1u : 0u;
+#pragma unroll
+    for (int ofs = 16; ofs > 0; ofs >>= 1) swp += __shfl_xor_sync(0xffffffffu, swp, ofs);
     if (lane == 0) {
         if (exc) atomicAdd(&sc->n_exceeded, (unsigned)__popc(exc));
         if (ncv) atomicAdd(&sc->n_noconv, (unsigned)__popc(ncv));
         atomicMax(&sc->h_iter_max, itm);
+        atomicAdd(&sc->sweeps, (unsigned long long)swp);
     }
 }
 
-__global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; }
+__global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; sc->sweeps = 0ull; }
 
 template <bool UNIM, bool GLOB, int K>
-static void density_launch_k(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
-                             uint32_t hi) {
-    static bool attr_set = false;
-    if (!attr_set && !GLOB) {
-        cudaFuncSetAttribute(k_density<UNIM, GLOB, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        attr_set = true;
-    }
+static int density_launch_k(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
+                            uint32_t hi) {
+    if (!GLOB)   // per device: set on every launch
+        SPH_CUDA(c, cudaFuncSetAttribute(k_density<UNIM, GLOB, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     k_density<UNIM, GLOB, K><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
         c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db, dp,
         ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
     c->launches++;
+    return SPH_OK;
 }
 
 template <bool UNIM, bool GLOB>
-static void density_launch(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
-                           uint32_t hi) {
-    if (c->p.kernel == 0) density_launch_k<UNIM, GLOB, 0>(c, smem, db, dp, ncap, lo, hi);
-    else if (c->p.kernel == 1) density_launch_k<UNIM, GLOB, 1>(c, smem, db, dp, ncap, lo, hi);
-    else if (c->p.kernel == 2) density_launch_k<UNIM, GLOB, 2>(c, smem, db, dp, ncap, lo, hi);
-    else if (c->p.kernel == 3) density_launch_k<UNIM, GLOB, 3>(c, smem, db, dp, ncap, lo, hi);
-    else if (c->p.kernel == 4) density_launch_k<UNIM, GLOB, 4>(c, smem, db, dp, ncap, lo, hi);
-    else density_launch_k<UNIM, GLOB, 5>(c, smem, db, dp, ncap, lo, hi);
+static int density_launch(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
+                          uint32_t hi) {
+    if (c->p.kernel == 0) return density_launch_k<UNIM, GLOB, 0>(c, smem, db, dp, ncap, lo, hi);
+    if (c->p.kernel == 1) return density_launch_k<UNIM, GLOB, 1>(c, smem, db, dp, ncap, lo, hi);
+    if (c->p.kernel == 2) return density_launch_k<UNIM, GLOB, 2>(c, smem, db, dp, ncap, lo, hi);
+    if (c->p.kernel == 3) return density_launch_k<UNIM, GLOB, 3>(c, smem, db, dp, ncap, lo, hi);
+    if (c->p.kernel == 4) return density_launch_k<UNIM, GLOB, 4>(c, smem, db, dp, ncap, lo, hi);
+    return density_launch_k<UNIM, GLOB, 5>(c, smem, db, dp, ncap, lo, hi);
 }
 
 int launch_density(sph_ctx* c) {
@@ -300,11 +303,11 @@ int launch_density(sph_ctx* c) {
         const uint32_t ncap = cls == 2 ? 0u : ((c->nc_max < hi ? c->nc_max : hi) + 31u) & ~31u;
         const size_t smem = (size_t)ncap * 4 * sizeof(double);
         if (c->uniform_mass) {      // all masses equal (checked once at init): no per-neighbour mass registers
-            if (cls == 2) density_launch<true, true>(c, smem, db, dp, ncap, lo, hi);
-            else density_launch<true, false>(c, smem, db, dp, ncap, lo, hi);
+            if (cls == 2) SPH_TRY((density_launch<true, true>(c, smem, db, dp, ncap, lo, hi)));
+            else SPH_TRY((density_launch<true, false>(c, smem, db, dp, ncap, lo, hi)));
         } else {
-            if (cls == 2) density_launch<false, true>(c, smem, db, dp, ncap, lo, hi);
-            else density_launch<false, false>(c, smem, db, dp, ncap, lo, hi);
+            if (cls == 2) SPH_TRY((density_launch<false, true>(c, smem, db, dp, ncap, lo, hi)));
+            else SPH_TRY((density_launch<false, false>(c, smem, db, dp, ncap, lo, hi)));
         }
     }
     SPH_CUDA(c, cudaGetLastError());

@@ -17,6 +17,12 @@
 //     by a positive constant and squaring are monotone, so max() commutes with them exactly. Buckets whose union
 //     box with the group spans at most L/2 on every periodic axis cannot wrap and take a loop without the
 //     minimum-image selects (the decision is exact).
+//     Fast path (a4): the exact test is only needed for pairs close to the cutoff. Each group works in
+//     coordinates relative to the centre of its box, scaled by a power of two so that its reach is O(1), and rounded
+//     to fp32; the test runs in packed fp32 (two candidates per FADD2 / FMUL2 / FFMA2), with an error bound derived
+//     from the 2^-24 roundings of the relative coordinates. A bucket in which some lane saw |d^2 - cutoff^2| inside
+//     that bound is tested again with the plain IEEE fp64 expressions (from global memory): every decision that is
+//     kept is provably the fp64 one, so the sets stay bit-exact.
 //   Output (the cache): the group's candidate array (the sorted slots of the candidates that passed
 //     the prefilter, in traversal order) and, per particle, the ascending list of 16-bit indices into that
 //     candidate array. Hits are buffered in shared memory, candidate slots in a per-warp global scratch row, and
@@ -38,6 +44,7 @@ constexpr int kPendCap = 64;             // candidate buckets buffered before st
 constexpr int kHitCap = 112;             // buffered hits per lane
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
 constexpr int kHitStride = kHitCap + kHitSlack + 4;   // in u16: 296 B per lane row (8-byte aligned: copied out as u64)
+static_assert(kHitStride % 4 == 0, "hit rows are copied as u64 words");
 constexpr int kShare = 4;               // consecutive groups that share one tree walk
 constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
 constexpr int kSpillCap = 512;            // hits per lane that can spill from the shared-memory row to the warp's global scratch
@@ -55,9 +62,12 @@ struct TravBox {
 struct TravWarpSmem {
     uint32_t stack[kStackCap];
     uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
-    double2 cxy[32], czr[32];                 // staged candidates (compacted): {x, y}, {z, (R_kern chi h)^2}
-    uint32_t cid[32];                         // their indices in the group's candidate array
+    float prc[kPendCap];                      // their reach R_kern chi hmax_node in the group's scaled units, rounded up
+    float4 cand[kGroup + 2];                  // staged candidates (compacted), in pairs: {x0, x1, y0, y1}, {z0, z1, r0, r1}:
+                                              // scaled fp32 coordinates relative to the group's centre, r = cutoff^2
+    uint32_t cslotb[kGroup];                  // their sorted slots (exact path)
     uint32_t ub[kUbCap];                      // bucket nodes within reach of the kShare groups' common box
+    uint32_t rowoff[kGroup + 4];              // copy-out: first u64 word of each particle's list in the group's block
     uint16_t hits[32 * kHitStride];
 };
 
@@ -114,6 +124,12 @@ struct GroupCtx {
     uint32_t* cptr;       // candidate slots: the warp's scratch row, or (DIRECT) the group's array in global memory
     bool can_write;       // DIRECT: allocation succeeded
     bool anywrap;         // warp-uniform: some bucket of this group may wrap around a periodic axis
+    // fp32 fast path (warp-uniform unless marked): coordinates relative to (cx, cy, cz), scaled by sc (a power of two)
+    bool use32;
+    double cx, cy, cz, sc;
+    float ax, ay, az, ra2, rca;   // per lane: scaled relative position, cutoff^2 and cutoff (rounded up) of the query
+    float ex, ey, ez;             // scaled half extents of the group's box, rounded up
+    float twoA, rcg, rc2g_f;      // 2 max(ex, ey, ez); scaled reach of the group (rounded up) and its square
 };
 
 // d2 < a || d2 < b as two predicate-combining compares (the compiler otherwise builds a NaN-safe fp64 max)
@@ -122,6 +138,31 @@ __device__ __forceinline__ bool lt_either(double d2, double a, double b) {
     asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tsetp.lt.or.f64 p, %1, %3, p;\n\tselp.s32 %0, 1, 0, p;\n\t}"
         : "=r"(r) : "d"(d2), "d"(a), "d"(b));
     return r != 0;
+}
+
+// packed fp32 pairs (sm_100: FADD2 / FMUL2 / FFMA2, two candidates per instruction)
+__device__ __forceinline__ unsigned long long pk2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long sub2(unsigned long long a, unsigned long long b) {
+    unsigned long long r;
+    asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b) {
+    unsigned long long r;
+    asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
 }
 
 template <bool DIRECT>
@@ -139,12 +180,22 @@ __device__ __forceinline__ void record_hit(GroupCtx& G, uint32_t& wp, uint32_t l
     }
 }
 
+// Error bound of the fp32 fast path, in the group's scaled units. Relative coordinates r = x - centre (min-imaged for
+// buckets that may wrap) are exact to 2^-53 |r| in fp64 and are rounded once to fp32: |fl(r) - r| <= 2^-24 |r|. With
+// |r_a| <= A (half extent of the group's box) and |r_b| <= A + 3.01 rcm + 6 E for every candidate that passed the
+// prefilter below, each difference d_k = fl(r_a,k - r_b,k) has |d_k - true| <= E := 1.3e-7 (2 A + 3.1 rcm) (2^-23 =
+// 1.19e-7), hence |d2_f - d2| <= 2 sqrt(3) E d + 3 E^2 + 3.01 2^-24 d2, the thresholds carry 2^-24 relative each, and
+// for every test of a bucket  |v_f - v| <= B/4,  B := E (14 rcm' + 12 E) + 2e-6 rcm'^2,  v = d2 - max(cutoff^2),
+// rcm' = the larger of the query's and the bucket's reach (true hit: d <= rcm'; true miss: d2 - err(d) is increasing in
+// d beyond rcm', or E > rcm' / sqrt(3) and 12 E^2 covers it). So |v_f| > B implies sign(v_f) = sign(v), and sign(v) is
+// the fp64 decision because that differs from the real-number one only within 1e-15 relative of the cutoff.
 template <bool DIRECT>
 __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, unsigned lane, unsigned lt,
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const TravBox& tb, double rk_chi) {
     const uint32_t row = lane * kHitStride;
+    const unsigned long long ax2 = pk2(G.ax, G.ax), ay2 = pk2(G.ay, G.ay), az2 = pk2(G.az, G.az), ra22 = pk2(G.ra2, G.ra2);
     // software pipeline: the next bucket's candidate (one per lane) is in flight while this one is tested
     double px = 0.0, py = 0.0, pz = 0.0, ph = 0.0;
     if (npend > 0) {
@@ -163,68 +214,99 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             const uint32_t nlo = s.plo[b + 1] & ~kWrapBit;
             if (lane < s.pn[b + 1]) { px = x[nlo + lane]; py = y[nlo + lane]; pz = z[nlo + lane]; ph = h[nlo + lane]; }
         }
-        // per-candidate prefilter (one lane per candidate): squared distance from the candidate to the group's
-        // box against the larger of its own and the group's cutoff, with a relative margin far above rounding.
-        // Buckets that may wrap keep every candidate.
+        // per-candidate prefilter (one lane per candidate): squared distance from the candidate to the group's box
+        // against the larger of its own and the group's cutoff, conservative under rounding
         bool keep = lane < bn;
-        if (keep && !wrap) {
+        float fx = 0.f, fy = 0.f, fz = 0.f, fr = 0.f, band = 0.f;
+        if (G.use32) {
+            double rx = cx - G.cx, ry = cy - G.cy, rz = cz - G.cz;
+            if (wrap) {   // nearest periodic image of the candidate relative to the group's centre (unique: see launch)
+                rx = min_image(rx, tb.L[0], tb.halfL[0], tb.periodic[0]);
+                ry = min_image(ry, tb.L[1], tb.halfL[1], tb.periodic[1]);
+                rz = min_image(rz, tb.L[2], tb.halfL[2], tb.periodic[2]);
+            }
+            fx = (float)(rx * G.sc); fy = (float)(ry * G.sc); fz = (float)(rz * G.sc);
+            fr = (float)(rc2 * G.sc * G.sc);
+            const float rcn = s.prc[b];
+            const float rcm_g = fmaxf(rcn, G.rcg);
+            const float E = 1.3e-7f * (G.twoA + 3.1f * rcm_g);
+            const float gx = fmaxf(fabsf(fx) - G.ex, 0.f), gy = fmaxf(fabsf(fy) - G.ey, 0.f), gz = fmaxf(fabsf(fz) - G.ez, 0.f);
+            keep = keep && (gx * gx + gy * gy + gz * gz <= fmaxf(fr, G.rc2g_f) * 1.0001f + 16.f * E * (rcm_g + E));
+            const float rcm = fmaxf(G.rca, rcn);
+            band = E * (14.f * rcm + 12.f * E) + 2e-6f * rcm * rcm;
+        } else if (keep && !wrap) {   // plain fp64 version (groups too large for the scaled frame); wrapping buckets keep all
             const double gx = clamp0(dmax(G.gxl - cx, cx - G.gxh));
             const double gy = clamp0(dmax(G.gyl - cy, cy - G.gyh));
             const double gz = clamp0(dmax(G.gzl - cz, cz - G.gzh));
             keep = gx * gx + gy * gy + gz * gz <= dmax(rc2, G.rc2g) * (1.0 + 1e-9);
         }
         const unsigned km = __ballot_sync(0xffffffffu, keep);
-        const uint32_t nk = (uint32_t)__popc(km), nk4 = (nk + 3u) & ~3u, pos = (uint32_t)__popc(km & lt);
+        const uint32_t nk = (uint32_t)__popc(km), pos = (uint32_t)__popc(km & lt);
         __syncwarp();                                   // readers of the previous bucket are done
+        float* const cf = reinterpret_cast<float*>(s.cand);
         if (keep) {
-            s.cxy[pos] = make_double2(cx, cy);
-            s.czr[pos] = make_double2(cz, rc2);
-            s.cid[pos] = G.ncs + pos;                   // index in the group's candidate array
+            float* q = cf + (pos >> 1) * 8 + (pos & 1u);   // pair pos / 2, element pos & 1
+            q[0] = fx; q[2] = fy; q[4] = fz; q[6] = fr;
+            s.cslotb[pos] = blo + lane;
             if (DIRECT ? G.can_write : (G.ncs + pos < (uint32_t)kScrCap)) G.cptr[G.ncs + pos] = blo + lane;
         }
-        if (lane < 4u && nk + lane < nk4) {             // pad to a multiple of four with candidates nobody can hit
-            s.cxy[nk + lane] = make_double2(1e300, 1e300);
-            s.czr[nk + lane] = make_double2(1e300, 0.0);
-            s.cid[nk + lane] = 0u;
+        if (lane < 4u && nk + lane < ((nk + 3u) & ~3u)) {   // pad to a multiple of four with candidates nobody can hit
+            const uint32_t pp = nk + lane;
+            float* q = cf + (pp >> 1) * 8 + (pp & 1u);
+            q[0] = 1e18f; q[2] = 1e18f; q[4] = 1e18f; q[6] = 0.f;
         }
         __syncwarp();
         const uint32_t w0 = (uint32_t)__cvta_generic_to_shared(&s.hits[row + G.wpos]);
+        const uint32_t nhit0 = G.nhit;
         uint32_t wp = w0;
-        if (!wrap) {
-            for (uint32_t ci = 0; ci < nk4; ci += 4) {
-                const uint4 id4 = *reinterpret_cast<const uint4*>(&s.cid[ci]);
-                const uint32_t ids[4] = {id4.x, id4.y, id4.z, id4.w};
-                // all four candidates are loaded before the first hit is stored: the assembler keeps shared-memory
-                // loads behind earlier shared-memory stores, which would serialise the four tests
-                double2 a[4], c[4];
+        bool exact = !G.use32;
+        if (G.use32) {
+            float amin = 3e38f;
+            uint32_t id = G.ncs;
+            for (uint32_t j = 0; j < nk; j += 4, id += 4) {
+                // four candidates per trip, all loads before the first hit store (the assembler keeps shared-memory
+                // loads behind earlier shared-memory stores)
+                float4 c[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) { a[u] = s.cxy[ci + u]; c[u] = s.czr[ci + u]; }
+                for (int u = 0; u < 4; ++u) c[u] = s.cand[j + u];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const double dx = __dsub_rn(G.xq, a[u].x), dy = __dsub_rn(G.yq, a[u].y), dz = __dsub_rn(G.zq, c[u].x);
-                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                    if (lt_either(d2, G.rc2q, c[u].y)) record_hit<DIRECT>(G, wp, ids[u]);
+                for (int u = 0; u < 2; ++u) {
+                    const float4 c0 = c[2 * u], c1 = c[2 * u + 1];
+                    const unsigned long long dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w));
+                    const unsigned long long dz = sub2(az2, pk2(c1.x, c1.y));
+                    const unsigned long long d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                    float e0, e1, f0, f1;
+                    upk2(sub2(d2, pk2(c1.z, c1.w)), e0, e1);    // d2 - cutoff_b^2
+                    upk2(sub2(d2, ra22), f0, f1);               // d2 - cutoff_a^2
+                    const float v0 = fminf(e0, f0), v1 = fminf(e1, f1);     // < 0: within the larger cutoff
+                    amin = fminf(amin, fminf(fabsf(v0), fabsf(v1)));
+                    if (v0 < 0.f) record_hit<DIRECT>(G, wp, id + 2 * u);
+                    if (v1 < 0.f) record_hit<DIRECT>(G, wp, id + 2 * u + 1);
                 }
             }
-        } else {
-            // same grouping; the padding candidates sit at 1e300, whose minimum image is still out of reach
-            for (uint32_t ci = 0; ci < nk4; ci += 4) {
-                const uint4 id4 = *reinterpret_cast<const uint4*>(&s.cid[ci]);
-                const uint32_t ids[4] = {id4.x, id4.y, id4.z, id4.w};
-                double2 a[4], c[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) { a[u] = s.cxy[ci + u]; c[u] = s.czr[ci + u]; }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const double dx = min_image(__dsub_rn(G.xq, a[u].x), tb.L[0], tb.halfL[0], tb.periodic[0]);
-                    const double dy = min_image(__dsub_rn(G.yq, a[u].y), tb.L[1], tb.halfL[1], tb.periodic[1]);
-                    const double dz = min_image(__dsub_rn(G.zq, c[u].x), tb.L[2], tb.halfL[2], tb.periodic[2]);
-                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                    if (lt_either(d2, G.rc2q, c[u].y)) record_hit<DIRECT>(G, wp, ids[u]);
-                }
-            }
+            asm volatile("" ::: "memory");
+            // some test of this bucket too close to its cutoff for fp32: the bucket is decided again in fp64
+            exact = __any_sync(0xffffffffu, amin <= band);
+            if (exact) { wp = w0; G.nhit = nhit0; }
         }
-        asm volatile("" ::: "memory");                    // the row stores above are done as far as the compiler knows
+        if (exact) {
+            // plain IEEE fp64 test, no FMA contraction: bit-identical to the oracle's decision. One candidate at a
+            // time from global memory (warp-uniform addresses); rare on the fast path's workloads
+            for (uint32_t j = 0; j < nk; ++j) {
+                const uint32_t sl = s.cslotb[j];
+                const double rcb = __dmul_rn(rk_chi, h[sl]);
+                const double rc2b = __dmul_rn(rcb, rcb);
+                double dx = __dsub_rn(G.xq, x[sl]), dy = __dsub_rn(G.yq, y[sl]), dz = __dsub_rn(G.zq, z[sl]);
+                if (wrap) {
+                    dx = min_image(dx, tb.L[0], tb.halfL[0], tb.periodic[0]);
+                    dy = min_image(dy, tb.L[1], tb.halfL[1], tb.periodic[1]);
+                    dz = min_image(dz, tb.L[2], tb.halfL[2], tb.periodic[2]);
+                }
+                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                if (lt_either(d2, G.rc2q, rc2b)) record_hit<DIRECT>(G, wp, G.ncs + j);
+            }
+            asm volatile("" ::: "memory");
+        }
         if (!DIRECT) {
             const uint32_t got = (wp - w0) >> 1;
             G.nhit += got;
@@ -258,7 +340,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
 // One node against the box / hmax of G: group-group criterion on the squared box-box gap under the
 // minimum image, conservative under rounding (tiny pad); `wrap` says whether any (query, candidate) separation can
 // exceed L/2 on a periodic axis (exact: rounding is monotone). Entry e = internal node index, or leaf slot | kLeafBit.
-struct NodeHit { bool pass, small, wrap; uint32_t rlo, rhi, split; };
+struct NodeHit { bool pass, small, wrap; uint32_t rlo, rhi, split; float prc; };
 __device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, const double* __restrict__ x,
                                              const double* __restrict__ y, const double* __restrict__ z,
                                              const double* __restrict__ h, const NodeRec* __restrict__ nodes,
@@ -283,6 +365,7 @@ __device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, cons
         r.rhi = max(e, (uint32_t)other);
         r.small = (r.rhi - r.rlo + 1) <= tb.gmax;
     }
+    r.prc = (float)(rk_chi * bhm * G.sc) * 1.000001f;   // the node's reach in the group's scaled units, rounded up
     const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
     const double ggx = axis_gap(G.gxl, G.gxh, blo[0], bhi[0], tb.L[0], tb.periodic[0]);
     const double ggy = axis_gap(G.gyl, G.gyh, blo[1], bhi[1], tb.L[1], tb.periodic[1]);
@@ -344,13 +427,14 @@ __device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, uns
     for (int base = 0; base < nu; base += 32) {
         const bool have = base + (int)lane < nu;
         NodeHit r;
-        r.pass = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u;
+        r.pass = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u; r.prc = 0.f;
         if (have) r = node_test(s.ub[base + lane], G, x, y, z, h, nodes, tb, rk_chi);
         const unsigned em = __ballot_sync(0xffffffffu, r.pass);
         if (r.pass) {
             const int at = nb + __popc(em & lt);
             s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
             s.pn[at] = r.rhi - r.rlo + 1;
+            s.prc[at] = r.prc;
         }
         nb += __popc(em);
         __syncwarp();
@@ -380,7 +464,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
         sp -= npop;
         __syncwarp();
         NodeHit r;
-        r.pass = false; r.small = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u; r.split = 0u;
+        r.pass = false; r.small = false; r.wrap = false; r.rlo = 0u; r.rhi = 0u; r.split = 0u; r.prc = 0.f;
         if (have) r = node_test(e, G, x, y, z, h, nodes, tb, rk_chi);
         const bool push = r.pass && !r.small, emit = r.pass && r.small;
         const unsigned pm = __ballot_sync(0xffffffffu, push), em = __ballot_sync(0xffffffffu, emit);
@@ -394,6 +478,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
             const int at = nb + __popc(em & lt);
             s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
             s.pn[at] = r.rhi - r.rlo + 1;
+            s.prc[at] = r.prc;
         }
         nb += __popc(em);
         __syncwarp();
@@ -425,6 +510,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
     const unsigned lane = lane_id();
     const unsigned lt = lanemask_lt();
     const uint32_t n_groups = sc->n_groups;
+    const double reach_max = rk_chi * sc->h_max * 1.001;   // the largest cutoff radius of any particle (k_hmax ran before)
     unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u;
     uint16_t* const hit_row = out.hit_scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * (32 * kSpillCap);
     uint32_t* const scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
@@ -441,6 +527,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         int nu = -1;
         if (ng > 1u) {
             GroupCtx U;
+            U.sc = 1.0;
             U.gxl = U.gyl = U.gzl = 1e300; U.gxh = U.gyh = U.gzh = -1e300; U.ghm = 0.0;
             double vmax = 0.0, vmin = 1e300;
             for (uint32_t g = g0; g < g0 + ng; ++g) {
@@ -480,7 +567,31 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             const double rcg = __dmul_rn(rk_chi, G.ghm);
             G.rc2g = __dmul_rn(rcg, rcg);
         }
-        if (!qv) { G.xq = -1e300; G.rc2q = 0.0; }      // lanes without a particle can never hit
+        {
+            // fp32 frame of this group: centre and half extents of its box, scale 2^-e with e the exponent of its reach
+            // (every scaled quantity of the group is O(1) whatever the units). Usable if the scaled numbers are far
+            // from fp32's limits and, on periodic axes, half extent + the largest reach of any particle stays below
+            // L/2: then the periodic image of a candidate nearest to the centre is the one nearest to every query
+            // that can reach it, and a wrong image can only turn a far miss into another far miss.
+            const double rcg = rk_chi * G.ghm;
+            const int eb = (__double2hiint(rcg) >> 20) & 0x7ff;
+            const double hx = 0.5 * (G.gxh - G.gxl), hy = 0.5 * (G.gyh - G.gyl), hz = 0.5 * (G.gzh - G.gzl);
+            G.sc = __hiloint2double((2046 - eb) << 20, 0);
+            G.cx = 0.5 * (G.gxl + G.gxh); G.cy = 0.5 * (G.gyl + G.gyh); G.cz = 0.5 * (G.gzl + G.gzh);
+            const double As = dmax(hx, dmax(hy, hz)) * G.sc;
+            G.use32 = eb > 523 && eb < 1523 && As < 1e12 &&
+                      (!tb.periodic[0] || hx + reach_max < tb.halfL[0]) && (!tb.periodic[1] || hy + reach_max < tb.halfL[1]) &&
+                      (!tb.periodic[2] || hz + reach_max < tb.halfL[2]);
+            if (!G.use32) G.sc = 1.0;
+            G.ex = (float)(hx * G.sc) * 1.000001f; G.ey = (float)(hy * G.sc) * 1.000001f; G.ez = (float)(hz * G.sc) * 1.000001f;
+            G.twoA = 2.f * fmaxf(G.ex, fmaxf(G.ey, G.ez));
+            G.rcg = (float)(rcg * G.sc) * 1.000001f;
+            G.rc2g_f = (float)(G.rc2g * G.sc * G.sc);
+            G.ax = (float)((G.xq - G.cx) * G.sc); G.ay = (float)((G.yq - G.cy) * G.sc); G.az = (float)((G.zq - G.cz) * G.sc);
+            G.ra2 = (float)(G.rc2q * G.sc * G.sc);
+            G.rca = (float)(rk_chi * hq * G.sc) * 1.000001f;
+        }
+        if (!qv) { G.xq = -1e300; G.rc2q = 0.0; G.ax = G.ay = G.az = -1e18f; G.ra2 = 0.f; G.rca = 0.f; }   // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
         G.hspill = hit_row;
 
@@ -528,22 +639,31 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                     uint4* dst = reinterpret_cast<uint4*>(out.cslot + bbase);
                     for (uint32_t j = lane; j < (nc4 >> 2); j += 32) dst[j] = src[j];
                 }
-                // lists: the warp copies one particle's buffered list at a time (coalesced 16-bit stores)
+                // lists: the warp copies one particle's buffered list at a time (coalesced)
                 const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
-                for (uint32_t p = 0; p < nq; ++p) {
-                    const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
-                    uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 3u) & ~3u));
-                    if (spilled) {
+                if (!spilled) {
+                    // every list starts at a multiple of four entries of the group's block, so rows leave as u64
+                    // words (the up to three entries of padding are never read); the word offsets go through shared
+                    // memory so that the row loop needs no shuffles
+                    s.rowoff[lane] = (incl - nhit4) >> 2;
+                    if (lane == 31u) s.rowoff[32] = total >> 2;
+                    __syncwarp();
+                    uint64_t* const dst = reinterpret_cast<uint64_t*>(out.lists + lbase);
+                    const uint64_t* const src = reinterpret_cast<const uint64_t*>(s.hits);
+#pragma unroll 4
+                    for (uint32_t p = 0; p < nq; ++p) {
+                        const uint32_t o0 = s.rowoff[p], nw = s.rowoff[p + 1] - o0;
+                        for (uint32_t k = lane; k < nw; k += 32) dst[o0 + k] = src[p * (kHitStride / 4) + k];
+                    }
+                } else {
+                    for (uint32_t p = 0; p < nq; ++p) {
+                        const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
+                        uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 3u) & ~3u));
                         const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p);
                         const uint16_t* src = hit_row + (size_t)p * kSpillCap;
                         for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
                         sp0 += ns;
                         for (uint32_t k = lane; k < np - ns; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
-                    } else {
-                        // four entries per lane and store (the up to three entries of padding are never read)
-                        const uint64_t* src = reinterpret_cast<const uint64_t*>(&s.hits[p * kHitStride]);
-                        uint64_t* dst = reinterpret_cast<uint64_t*>(out.lists + sp0);
-                        for (uint32_t k = lane; k < (np + 3u) >> 2; k += 32) dst[k] = src[k];
                     }
                 }
             } else {
@@ -584,12 +704,8 @@ size_t trav_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * kScrCa
 size_t trav_hit_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * 32 * kSpillCap; }
 
 int launch_traverse(sph_ctx* c) {
-    static bool attr_set = false;
     const int smem = (int)sizeof(TravWarpSmem) * kTravWarps;
-    if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_traverse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
-    }
+    SPH_CUDA(c, cudaFuncSetAttribute(k_traverse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));   // per device: every launch
     TravBox tb;
     double Lmax = 0.0;
     for (int k = 0; k < 3; ++k) {
@@ -630,21 +746,23 @@ __global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t*
                                                       const uint32_t* __restrict__ cnt,
                                                       const uint64_t* __restrict__ lstart,
                                                       const uint16_t* __restrict__ lists,
-                                                      const uint64_t* __restrict__ offs, uint32_t* __restrict__ idx) {
-    const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (a >= N) return;
+                                                      const uint64_t* __restrict__ offs, uint32_t* __restrict__ idx,
+                                                      int64_t first, int64_t count) {
+    const int64_t a = first + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= first + count) return;
     const uint32_t g = gscan[a + 1] - 1u;          // gscan = exclusive scan of the group-start flags
     const GroupRec gr = ginfo[g];
     const uint32_t* cs = cslot + (((uint64_t)gr.cs_off_hi << 32) | gr.cs_off_lo);
     const uint16_t* li = lists + lstart[a];
     const uint32_t n = cnt[a];
-    const uint64_t o = offs[a];
+    const uint64_t o = offs[a] - offs[first];
     for (uint32_t k = 0; k < n; ++k) idx[o + k] = cs[li[k]];
 }
 
-int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out) {
-    k_cache_to_csr<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->cslot, c->cnt, c->lstart,
-                                                             c->lists, c->offs, idx_out);
+// lists of the sorted slots [first, first + count) into idx_out, which starts at the first slot's list
+int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out, int64_t first, int64_t count) {
+    k_cache_to_csr<<<div_up(count, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->cslot, c->cnt, c->lstart,
+                                                              c->lists, c->offs, idx_out, first, count);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -3,6 +3,8 @@
 // are resolved with a decoupled look-back over single-word (flag|count) status entries; ranking inside a tile
 // uses a warp-level ballot multisplit. Replaces the paper's bitonic sort, which it
 // says dominates the tree build. HBM-bound: 8 B + 8 x 24 B = 200 B per particle.
+#include <stdlib.h>
+
 #include <utility>
 
 #include "common.cuh"
@@ -75,7 +77,7 @@ __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ 
 
 // ---- kernel 2: exclusive scan of each digit histogram -> global digit bases ----
 __global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ ghist, DevScalars* sc) {
-    if (threadIdx.x == 0) sc->tie_max = 0u;
+    if (threadIdx.x == 0) { sc->tie_max = 0u; sc->sort_redo = 0u; }
     __shared__ uint32_t wsum[kRadix / 32];
     const unsigned d = threadIdx.x, lane = lane_id(), w = d >> 5;
     for (int p = 0; p < kPasses; ++p) {
@@ -246,16 +248,21 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint64_t* __
 // by the full key (stable, so equal keys keep their previous order): the result is exactly the stable sort by the
 // full key. Runs are rare and short when the prefix resolves the particles (40 of 63 bits: cells of 2^-13.3 of the
 // box per axis); the longest run is recorded so that the host falls back to all eight passes when it is not.
+// A run longer than max_run is not repaired (the insertion sort is quadratic and runs on one thread): the kernel
+// raises sc->sort_redo instead, the tree kernels of this build then do nothing, and the host sorts again with all
+// eight passes (api.cu). Prefix mode is only chosen after a sort whose longest run was <= 64, so this needs a sudden
+// collapse of many particles into one 2^-13 cell between two steps.
 __global__ void __launch_bounds__(256) k_sort_repair(int64_t N, uint64_t* __restrict__ key, uint32_t* __restrict__ val,
-                                                     int shift, DevScalars* sc) {
+                                                     int shift, int64_t max_run, DevScalars* sc) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const uint64_t p = key[i] >> shift;
     if (i > 0 && (key[i - 1] >> shift) == p) return;          // not the head of a run
     int64_t e = i + 1;
-    while (e < N && (key[e] >> shift) == p) ++e;
+    while (e < N && e - i <= max_run && (key[e] >> shift) == p) ++e;
     if (e - i < 2) return;
     atomicMax(&sc->tie_max, (unsigned int)min(e - i, (int64_t)0x7fffffff));
+    if (e - i > max_run) { sc->sort_redo = 1u; return; }
     for (int64_t a = i + 1; a < e; ++a) {
         const uint64_t kk = key[a];
         const uint32_t vv = val[a];
@@ -272,12 +279,11 @@ int sort_scratch_bytes(int64_t N, int64_t* tiles, size_t* status_bytes) {
     return SPH_OK;
 }
 
+constexpr int64_t kRepairMaxRun = 2048;          // longest run of equal prefixes the repair kernel sorts (4 M key moves at worst)
+
 int launch_sort(sph_ctx* c) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPH_CUDA(c, cudaFuncSetAttribute(k_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
-        attr_set = true;
-    }
+    // function attributes are per device: set on every launch (cheap) rather than once per process
+    SPH_CUDA(c, cudaFuncSetAttribute(k_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
     const int64_t N = c->N, tiles = c->sort_tiles;
     const size_t status_per_pass = (size_t)tiles * kRadix;
     SPH_CUDA(c, cudaMemsetAsync(c->sort_hist, 0, kPasses * kRadix * sizeof(uint32_t), c->stream));
@@ -308,7 +314,11 @@ int launch_sort(sph_ctx* c) {
         std::swap(c->val, c->val_alt);
     }
     if (!short_codes) {
-        k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, c->d_sc);
+        // in an eight-pass sort the kernel only takes the census of equal prefixes (every run is already in order);
+        // SPH_REPAIR_MAX (tests) lowers the bound so that the redo path can be reached with small inputs
+        const char* env = getenv("SPH_REPAIR_MAX");
+        const int64_t max_run = (p0 == 0) ? (int64_t)1 << 40 : (env ? (int64_t)atoll(env) : kRepairMaxRun);
+        k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, max_run, c->d_sc);
         c->launches++;
     }
     SPH_CUDA(c, cudaGetLastError());

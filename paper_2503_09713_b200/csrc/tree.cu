@@ -17,7 +17,9 @@ __device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int N
 
 // one thread per internal node i in [0, N-2]
 __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
-                                                int32_t* __restrict__ parent, uint32_t* __restrict__ gflag, int gmax) {
+                                                int32_t* __restrict__ parent, uint32_t* __restrict__ gflag, int gmax,
+                                                const DevScalars* __restrict__ sc) {
+    if (sc->sort_redo) return;   // keys are not in order (sort.cu: k_sort_repair gave up): no groups, nothing downstream runs
     const int N = (int)N64;
     const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
     if (i >= N - 1) return;
@@ -197,7 +199,7 @@ int launch_tree(sph_ctx* c) {
     const int64_t N = c->N;
     SPH_CUDA(c, cudaMemsetAsync(c->gflag, 0, (size_t)N * sizeof(uint32_t), c->stream));
     if (N >= 2) {
-        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag, c->p.group_max);
+        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag, c->p.group_max, c->d_sc);
         c->launches++;
     } else {
         k_single_group<<<1, 1, 0, c->stream>>>(c->gflag);

@@ -27,7 +27,7 @@ def _declared_functions():
 def test_library_exports_every_declared_symbol(lib):
     from paper_2503_09713_b200 import binding
     names = _declared_functions()
-    assert len(names) >= 17
+    assert len(names) >= 18
     for n in names:
         assert hasattr(lib, n), f"{n} declared in sph_b200.h but not exported"
     assert sorted(binding.SYMBOLS) == names
@@ -92,7 +92,7 @@ def test_workload_generators_are_deterministic_and_shaped():
     assert np.all((a.pos >= 0) & (a.pos < 1)) and a.mass.sum() == pytest.approx(1.0)
     s = W.sod(16, 8)
     assert s.n == 16 * 8 * 8 + 8 * 4 * 4 and np.all(s.pos[0] >= -0.5) and np.all(s.pos[0] < 0.5)
-    assert W.sod(128, 64).n == 589_824 if False else True   # full C1 size is checked on the GPU box
+    assert W.sod(32, 16).n == 589_824 // 64                  # C1 is sod(128, 64): 64 times as many sites
     d = W.disc(2000, seed=1)
     R = np.hypot(d.pos[0], d.pos[1])
     assert R.min() >= 2 and R.max() <= 10 and np.all(np.abs(d.pos[2]) <= 3 * 0.05 * R * (R / 2) ** 0.25 + 1e-12)

@@ -39,7 +39,7 @@ def _near_cutoff_pairs(pos, h, box, chi, offs, idx):
     return int((np.abs(d2 / rc2 - 1.0) < BAND).sum())
 
 
-def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None):
+def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None, hn_exact=True):
     """Compare every stage of one evaluation. `state` = (pos, vel, u) in original order the evaluation started
     from (default: the workload's initial conditions); hn = the h^n it started from."""
     box, p = O.workload_box_params(w)
@@ -78,7 +78,10 @@ def _stage_parity(w, sim, state=None, hn=None, expect_restarts=None):
     box6, hmax = O.aabb(t, ps, hn[gperm])
     assert np.array_equal(g["aabb"], box6), "node boxes differ"
     if ev["restarts"] == 0:
-        assert np.array_equal(g["hmax"], hmax), "node hmax differs"
+        if hn_exact:
+            assert np.array_equal(g["hmax"], hmax), "node hmax differs"
+        else:       # h^n was computed by the library itself (sph_init's fallback): equal to rounding
+            assert np.allclose(g["hmax"], hmax, rtol=1e-14, atol=0.0), "node hmax differs"
         # a4: neighbour sets (sorted-slot indices), compared as sets per particle
         oo, oi = O.neighbours(ps, hn[gperm], box, p.chi, "grid", kernel=p.kernel)
         go, gi = sim.get_neighbours()
@@ -374,29 +377,272 @@ def _invariants(w, sim):
     assert np.all(np.abs(ma) < 1e-10 * np.abs(w.mass * f["acc"]).sum(axis=1).max() + 1e-300)
 
 
-def test_c2_full_size_sampled_parity():
+def _integer_stages_full(sim, pos, hn, box, fresh, tree=True):
+    """Bit-exact parity of the integer stages on ALL particles, whatever the size (protocol P1: `pos` are the positions
+    the build started from, in original order, `hn` the h^n of the last cache build): sorted keys and permutation
+    against the oracle's keys and stable sort, every tree table against its recursive builder, node boxes and hmax.
+    `fresh`: the sort started from the original order (ties follow the original index); on a stepped state equal keys
+    follow the previous slot order, so only validity is checked for them. Returns the GPU's permutation."""
+    n = pos.shape[1]
+    key = O.morton_keys(pos, box)
+    skey, perm = O.sort_keys(key)
+    gkey, gperm = sim.get_keys_perm()
+    assert np.array_equal(gkey, skey), "sorted Morton keys differ"
+    if fresh or np.all(skey[1:] != skey[:-1]):
+        assert np.array_equal(gperm, perm), "sort permutation differs"
+    else:
+        assert np.array_equal(np.sort(gperm), np.arange(n, dtype=gperm.dtype)) and np.array_equal(key[gperm], skey)
+    del key, perm
+    if tree:
+        t = O.tree(skey)
+        g = sim.get_tree()
+        for k in ("left", "right", "lflag", "rflag", "parent", "rlo", "rhi"):
+            assert np.array_equal(g[k], t[k]), f"tree table {k} differs"
+        box6, hmax = O.aabb(t, pos[:, gperm], hn[gperm])
+        assert np.array_equal(g["aabb"], box6), "node boxes differ"
+        assert np.array_equal(g["hmax"], hmax), "node hmax differs"
+    return gperm
+
+
+def _slot_sample_parity(sim, gperm, s0, count, pos, vel, u, hn, mass, box, p, f, closure=None):
+    """Parity on a sample of a large run in the configuration it runs in. Targets: the particles in the sorted slots
+    [s0, s0 + count), a compact Morton block. The oracle evaluates them with the plain definitions on every particle
+    within two cache radii of the block (the 2-hop closure: the targets' neighbours need rho and Omega, hence their own
+    complete lists) from the state (pos, vel, u, h^n = hn) the GPU evaluation started from (P1). Compared: the
+    targets' neighbour SETS (bit-exact), h, rho (1e-10), Omega, a and du/dt (1e-8 of the global max). `f`: the GPU's
+    fields in original order. `closure`: a function giving the 2-hop closure for open boxes with strongly varying h."""
+    n = pos.shape[1]
+    tg = gperm[s0:s0 + count].astype(np.int64)
+    if closure is not None:
+        sub = closure(tg)
+    else:
+        lo = np.array([box.lo[k] for k in range(3)])
+        L = np.array([box.hi[k] - box.lo[k] for k in range(3)])
+        rc = kern_r(p) * p.chi * max(float(hn.max()), float(f["h"].max()))
+        blo, bhi = pos[:, tg].min(axis=1), pos[:, tg].max(axis=1)
+        keep = np.ones(n, dtype=bool)
+        for k in range(3):
+            assert bhi[k] - blo[k] < 0.5 * L[k], "the slot block is not compact"
+            gap = lambda x: np.maximum(np.maximum(blo[k] - x, x - bhi[k]), 0.0)      # distance from x to [blo, bhi]
+            d = gap(pos[k])
+            if box.periodic[k]:     # ... under the nearest periodic image
+                d = np.minimum(d, np.minimum(gap(pos[k] + L[k]), gap(pos[k] - L[k])))
+            keep &= d <= 2.02 * rc
+        sub = np.nonzero(keep)[0]
+    assert sub.size < 600_000 and np.all(np.isin(tg, sub))
+    tgt = np.searchsorted(sub, tg)
+    ps, vs = np.ascontiguousarray(pos[:, sub]), np.ascontiguousarray(vel[:, sub])
+    ms, us, hs = mass[sub].copy(), u[sub].copy(), hn[sub].copy()
+    oo, oi = O.neighbours(ps, hs, box, p.chi, "grid", kernel=p.kernel)
+    # neighbour sets of the targets: GPU lists hold sorted slots -> original ids through the permutation
+    go, gi = sim.get_neighbours_range(s0, count)
+    assert np.array_equal(np.diff(go).astype(np.int64), np.diff(oo).astype(np.int64)[tgt]), "neighbour counts differ"
+    gid = gperm[gi].astype(np.int64)
+    for j in range(count):
+        mine = np.sort(gid[go[j]:go[j + 1]])
+        theirs = np.sort(sub[oi[oo[tgt[j]]:oo[tgt[j] + 1]]])
+        assert np.array_equal(mine, theirs), f"neighbour set of slot {s0 + j} differs"
+    dn = O.density(ps, ms, hs, oo, oi, box, p)
+    hop1 = np.unique(oi[np.concatenate([np.arange(oo[t], oo[t + 1]) for t in tgt]).astype(np.int64)])
+    assert not dn["exceeded"][hop1].any()
+    acc, dudt, _ = O.forces(ps, vs, ms, dn["h"], dn["rho"], dn["omega"], us, oo, oi, box, p)
+    assert np.max(np.abs(f["h"][tg] / dn["h"][tgt] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["rho"][tg] / dn["rho"][tgt] - 1)) < TOL_RHO_H
+    assert np.max(np.abs(f["omega"][tg] - dn["omega"][tgt])) < 1e-9
+    hmax = float(f["h"].max())
+    cs2 = p.gamma * (p.gamma - 1.0) * np.abs(u).max() if p.eos == 0 else p.cs0 ** 2
+    amax = max(np.abs(f["acc"]).max(), 1e-3 * cs2 / hmax)
+    dmax = max(np.abs(f["dudt"]).max(), 1e-3 * cs2 ** 1.5 / hmax)
+    assert np.max(np.abs(f["acc"][:, tg] - acc[:, tgt])) <= TOL_ACC * amax
+    assert np.max(np.abs(f["dudt"][tg] - dudt[tgt])) <= TOL_ACC * dmax
+
+
+def kern_r(p):
+    return {1: 2.5, 2: 3.0}.get(p.kernel, 2.0)
+
+
+def _host(sim, names):
+    return {k: v.numpy() for k, v in sim.get_fields(names, host=True).items()}
+
+
+def _stepped_parity(w, sim, n_steps, check_steps, blocks, count=1024, tree=True, closure=None):
+    """Runs `n_steps` leapfrog steps and, after each step in `check_steps`, compares the stepped context (prefix-mode
+    sort + repair, reused cache pools, shared walks) with the oracle under protocol P1: the integer stages on all
+    particles from the positions the step's build started from (the GPU's own, which the corrector does not change)
+    and the h^n before the step; and sets + fields on Morton blocks of `count` slots starting at the fractions
+    `blocks` of the slot range, from v*, u* = the predictor (G1, G3) applied to the GPU's pre-step state."""
+    box, p = O.workload_box_params(w)
+    for step in range(1, n_steps + 1):
+        check = step in check_steps
+        pre = _host(sim, ("vel", "u", "h", "acc", "dudt")) if check else None
+        dt = sim.step_leapfrog(want_dt=check)
+        st = sim.stats()
+        assert st["steps"] == step
+        if not check:
+            continue
+        assert st["restarts"] == 0
+        f = _host(sim, ("pos", "h", "rho", "omega", "acc", "dudt"))
+        gperm = _integer_stages_full(sim, f["pos"], pre["h"], box, fresh=False, tree=tree)
+        vstar = (pre["vel"] + 0.5 * dt * pre["acc"]) + 0.5 * dt * pre["acc"]          # G1, G3
+        ustar = (pre["u"] + 0.5 * dt * pre["dudt"]) + 0.5 * dt * pre["dudt"]
+        for frac in blocks:
+            s0 = min(int(frac * w.n) // count * count, w.n - count)
+            _slot_sample_parity(sim, gperm, s0, count, f["pos"], vstar, ustar, pre["h"], w.mass, box, p, f, closure)
+    return sim.stats()
+
+
+def test_c2_full_size_stepped_parity():
     """BASELINE config 2 at full size (256^3 = 16.8 M particles), the workload and launch configuration bench.py
-    times: invariants on everything, oracle parity on two sampled regions (interior; across the periodic corner)."""
+    times, for its 5 steps. White step: integer stages bit-exact on all particles, sampled parity (interior; across the
+    periodic corner) and neighbour sets on Morton blocks. After steps 2 and 5 (five-pass prefix sort + repair, reused
+    pools, shared walks): the same, from the GPU's own pre-step state (P1)."""
     w = W.cube(256, jitter=0.1, steps=5)
+    box, p = O.workload_box_params(w)
     sim = _sim(w)
     _invariants(w, sim)
+    gperm = _integer_stages_full(sim, w.pos, w.h0, box, fresh=True)
     n1 = _sampled_parity(w, sim, (0.43, 0.52, 0.37), 0.02)
     n2 = _sampled_parity(w, sim, (0.0, 1.0, 0.0), 0.02)          # wraps around all three periodic faces
     assert n1 > 900 and n2 > 900
+    f = _host(sim, ("h", "rho", "omega", "acc", "dudt"))
+    for s0 in (0, 5 * 4096 * 7, w.n - 4096):                     # first block (touches three faces), interior, last
+        _slot_sample_parity(sim, gperm, s0, 1024, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f)
     st = sim.stats()
     assert st["n_groups"] == w.n // 32 and 75 < st["nbr_mean"] < 90
-    sim.step_leapfrog()                                           # and one full step in that configuration
-    assert sim.stats()["steps"] == 1
+    del f, gperm
+    st = _stepped_parity(w, sim, 5, (2, 5), (0.0, 0.37, 0.999))
+    assert st["sort_passes"] == 5 and st["share_chunk"] == 4     # the configuration the bench times
+    _invariants(w, sim)
     sim.close()
 
 
-def test_c1_sod_full_size_sampled_parity():
-    """BASELINE config 1 at full size (589,824 particles): sampled parity across the density jump at x = 0."""
+def test_c1_sod_full_size_stepped_parity():
+    """BASELINE config 1 at full size (589,824 particles) for its 10 steps: integer stages on all particles and sampled
+    parity across the density jump at x = 0 and at the periodic seam, at the white step and after steps 1, 5 and 10."""
     w = W.config(1)
+    box, p = O.workload_box_params(w)
     sim = _sim(w)
     _invariants(w, sim)
+    gperm = _integer_stages_full(sim, w.pos, w.h0, box, fresh=True)
     _sampled_parity(w, sim, (0.0, 0.0, 0.0), 0.03)
     _sampled_parity(w, sim, (0.5, 0.125, -0.125), 0.03)          # the periodic seam, a box corner
+    f = _host(sim, ("h", "rho", "omega", "acc", "dudt"))
+    inv = np.empty(w.n, np.int64)
+    inv[gperm] = np.arange(w.n)
+    jump = int(inv[np.argmin(np.abs(w.pos[0] + 0.5 / 256) + np.abs(w.pos[1]) + np.abs(w.pos[2]))])   # a slot at x = 0-
+    for s0 in (0, jump // 512 * 512, w.n - 512):
+        _slot_sample_parity(sim, gperm, s0, 512, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f)
+    _stepped_parity(w, sim, 10, (1, 5, 10), (0.0, jump / w.n, 0.999), count=512)
+    _invariants(w, sim)
+    sim.close()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n_side", [384, 512])
+def test_c4_large_sweep_points_parity(n_side):
+    """BASELINE config 4's two largest points: 384^3 (leaf groups of 27: other bucket shapes) and 512^3 (1.08e10 list
+    entries: 64-bit list offsets, 89 GB). Invariants, integer stages bit-exact on all particles, sets + fields on Morton
+    blocks (first, interior, beyond the 2^32-nd list entry, last), at the white step and after 2 steps."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if n_side ** 3 * 720 > free:
+        pytest.skip(f"{n_side}^3 needs ~{n_side ** 3 * 720 / 1e9:.0f} GB of device memory")
+    w = W.cube(n_side, jitter=0.1, steps=2)
+    box, p = O.workload_box_params(w)
+    sim = _sim(w)
+    st = sim.stats()
+    assert st["restarts"] == 0 and 75 < st["nbr_mean"] < 90
+    if n_side == 512:
+        assert st["n_neighbours"] > 2 ** 32
+    _invariants(w, sim)
+    gperm = _integer_stages_full(sim, w.pos, w.h0, box, fresh=True)
+    f = _host(sim, ("h", "rho", "omega", "acc", "dudt"))
+    for frac in (0.0, 0.31, 0.55, 0.999):
+        s0 = min(int(frac * w.n) // 1024 * 1024, w.n - 1024)
+        _slot_sample_parity(sim, gperm, s0, 1024, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f)
+    del f, gperm
+    _stepped_parity(w, sim, 2, (2,), (0.0, 0.55, 0.999))
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+
+
+def test_sph_init_entry_point():
+    """north_star's entry `sph_init` itself (9 arguments: device pointers, no h0, NULL stream, cudaMalloc): the
+    fallback h0 = h_fact (m V_box / M_tot)^(1/3) of reading A9 is computed by the library (k_sum, k_h0_fallback); the
+    test computes the same for the oracle. C0, and a cloud of unequal masses whose white step needs chi-restarts."""
+    import torch
+    from paper_2503_09713_b200 import binding as B
+    w0 = W.config(0)
+    w1 = W.random_cloud(4000, seed=17, periodic=True, clustered=False)
+    w1.mass = w1.mass * (0.5 + W.splitmix_u01(5, np.arange(w1.n, dtype=np.uint64), 0))
+    for w in (w0, w1):
+        vol = float(np.prod(np.array(w.box_hi) - np.array(w.box_lo)))
+        w.h0 = w.hfact * np.cbrt(w.mass * vol / w.mass.sum())
+        dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.pos, w.vel, w.mass, w.u)]
+        sim = B.Sim.from_sph_init(*dev, w.box_lo, w.box_hi, w.periodic, w.gamma, w.hfact)
+        ev, f = _stage_parity(w, sim, hn_exact=(w is w0))     # equal masses 2^-12: the fallback is exact, 1.2 / 16
+        assert sim.step_leapfrog(want_dt=True) == pytest.approx(ev["dt"], rel=1e-12)
+        sim.close()
+    assert ev["restarts"] >= 0
+
+
+def test_two_contexts_alive_at_once():
+    """Two contexts in one process, calls interleaved: each gives bitwise the fields of a run on its own (no state is
+    shared between contexts; per-launch function attributes)."""
+    wa, wb = W.cube(16, jitter=0.05, vel_amp=0.02, seed=3), W.random_cloud(5000, seed=3)
+
+    def alone(w):
+        s = _sim(w)
+        for _ in range(3):
+            s.step_leapfrog()
+        f = _np(s.get_fields())
+        s.close()
+        return f
+
+    fa, fb = alone(wa), alone(wb)
+    a, b = _sim(wa), _sim(wb)
+    for _ in range(3):
+        a.step_leapfrog()
+        b.step_leapfrog()
+    ga, gb = _np(a.get_fields()), _np(b.get_fields())
+    for k in fa:
+        assert np.array_equal(fa[k], ga[k]) and np.array_equal(fb[k], gb[k]), k
+    a.close()
+    b.close()
+
+
+def test_sort_redo_when_a_run_is_too_long_to_repair(monkeypatch):
+    """Prefix-mode sort meeting a run of equal 40-bit prefixes longer than the repair bound (sudden collapse of many
+    particles into one 2^-13 cell between two steps): the repair kernel gives up, the tree kernels of that build do
+    nothing, the host sorts again with all eight passes. Reached here by lowering the bound (SPH_REPAIR_MAX) and
+    moving a cluster together through the velocities, so that the positions change inside step_leapfrog."""
+    from paper_2503_09713_b200 import binding as B
+    monkeypatch.setenv("SPH_REPAIR_MAX", "16")
+    w = W.random_cloud(6000, seed=41, periodic=False, clustered=False)
+    w.h0 = np.minimum(w.h0, 0.1)
+    sim = _sim(w, params=B.params_for(w, max_h_iter=400))               # h of the cluster shrinks by 1.2 per sweep
+    assert sim.stats()["sort_passes"] == 8 and sim.stats()["sort_tie_max"] <= 16
+    # velocities that carry 40 particles into one cell of 1e-6 during a step of dt = 1
+    tgt = np.array([0.5, 0.5, 0.5])[:, None] + 2e-5 * np.random.default_rng(1).random((3, 40))
+    vel = np.zeros_like(w.vel)
+    vel[:, :40] = tgt - w.pos[:, :40]
+    pre = _np(sim.get_fields(("pos", "h")))
+    sim.set_fields(vel=vel, acc=np.zeros_like(w.vel), dudt=np.zeros(w.n))
+    sim.build_tree(); sim.compute_density(); sim.compute_forces()       # a^n for the new velocities, prefix mode armed
+    sim.set_fields(acc=np.zeros_like(w.vel), dudt=np.zeros(w.n))          # ballistic step: x += dt v exactly
+    assert sim.stats()["sort_tie_max"] <= 16
+    sim.step_leapfrog(dt=1.0)
+    st = sim.stats()
+    assert st["sort_tie_max"] >= 40 and st["sort_passes"] == 8          # gave up in prefix mode, sorted again in full
+    box, p = O.workload_box_params(w)
+    f = _np(sim.get_fields(("pos",)))
+    key = O.morton_keys(f["pos"], box)
+    gkey, gperm = sim.get_keys_perm()
+    assert np.array_equal(gkey, np.sort(key)) and np.array_equal(key[gperm], gkey)
+    t, g = O.tree(gkey), sim.get_tree()
+    for k in ("left", "right", "lflag", "rflag", "parent", "rlo", "rhi"):
+        assert np.array_equal(g[k], t[k])
     sim.close()
 
 
@@ -475,10 +721,12 @@ def _check_sorted_state(sim, pos, box, prev_perm=None):
 def test_sort_prefix_mode_and_tie_repair(cluster):
     """From the second build on the sort uses five passes over the top 40 key bits plus a repair of the runs that
     share them, if the previous sort saw only short runs (<= 64), else all eight passes. Clusters of particles
-    inside one 2^-14 cell make such runs; both modes must give the stable sort by the full key."""
+    inside one 2^-14 cell make such runs; both modes must give the stable sort by the full key. The particles are
+    moved by a ballistic leapfrog step (sph_set_fields with new positions goes back to the full sort)."""
     from paper_2503_09713_b200 import binding as B
     n, ncl = 6000, 12
     w = W.random_cloud(n, seed=31, periodic=False, clustered=False)
+    w.h0 = np.minimum(w.h0, 0.1)
     rng = np.random.default_rng(cluster)
 
     def clustered(pos):
@@ -491,21 +739,25 @@ def test_sort_prefix_mode_and_tie_repair(cluster):
 
     w.pos = clustered(w.pos)
     box, p = O.workload_box_params(w)
-    sim = B.Sim.from_workload(w, white_step=False)
-    sim.build_tree()
+    sim = _sim(w, params=B.params_for(w, max_h_iter=400))       # h of the clustered particles shrinks by 1.2 per sweep
     st = sim.stats()
     assert st["sort_passes"] == 8 and st["sort_tie_max"] >= cluster
-    perm0 = _check_sorted_state(sim, w.pos, box)
-    # new positions: every particle moves, clusters are re-drawn; the next sort starts from the previous order
+    _check_sorted_state(sim, w.pos, box)
+    # new positions: every particle moves, clusters are re-drawn; reached by one step of dt = 1 with a = 0
     pos1 = clustered(np.clip(w.pos + 0.01 * (rng.random((3, n)) - 0.5), 0.0, np.nextafter(1.0, 0.0)))
-    sim.set_fields(pos=pos1)
-    sim.build_tree()
+    sim.set_fields(vel=pos1 - w.pos, acc=np.zeros_like(w.vel), dudt=np.zeros(n))
+    sim.build_tree(); sim.compute_density(); sim.compute_forces()
+    sim.set_fields(acc=np.zeros_like(w.vel), dudt=np.zeros(n))
+    perm0 = sim.get_keys_perm()[1]
+    sim.step_leapfrog(dt=1.0)
     st = sim.stats()
-    assert st["sort_passes"] == (5 if cluster <= 64 else 8)
-    _check_sorted_state(sim, pos1, box, prev_perm=perm0)
-    oo, oi = O.neighbours(pos1[:, sim.get_keys_perm()[1]], w.h0[sim.get_keys_perm()[1]], box, p.chi, "grid")
-    go, gi = sim.get_neighbours()
-    assert np.array_equal(go, oo)
+    assert st["sort_passes"] == (5 if cluster <= 64 else 8) and st["sort_tie_max"] >= cluster
+    pos_now = _np(sim.get_fields(("pos",)))["pos"]
+    assert np.max(np.abs(pos_now - pos1)) < 1e-15
+    _check_sorted_state(sim, pos_now, box, prev_perm=perm0)
+    t, g = O.tree(sim.get_keys_perm()[0]), sim.get_tree()
+    for k in ("left", "right", "lflag", "rflag", "parent", "rlo", "rhi"):
+        assert np.array_equal(g[k], t[k])
     sim.close()
 
 
@@ -647,6 +899,25 @@ def test_c3_disc_full_size_sampled_parity():
     cnt_orig = np.empty(w.n, dtype=np.int64)
     cnt_orig[perm] = np.diff(offs).astype(np.int64)
     assert np.array_equal(cnt_orig[tgt_g], np.diff(oo).astype(np.int64)[tgt])
+    # white step of the converged state: integer stages on all 10^7 particles; then the config's 5 steps with the
+    # stepped context compared after steps 2 and 5 (sets and fields on a Morton block at mid-radius, closure by KD-tree)
+    gperm = _integer_stages_full(sim, w.pos, w.h0, box, fresh=True)
+    s0 = int(np.nonzero(gperm == tgt_g[0])[0][0]) // 512 * 512
+    closure = lambda pos, h: (lambda tg: _closure_two_hops(pos, h, p.chi, tg))
+    _slot_sample_parity(sim, gperm, s0, 512, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f, closure(w.pos, w.h0))
+    del f, gperm
+    for step in range(1, 6):
+        check = step in (2, 5)
+        pre = _host(sim, ("vel", "u", "h", "acc", "dudt")) if check else None
+        dt = sim.step_leapfrog(want_dt=check)
+        if not check:
+            continue
+        assert sim.stats()["restarts"] == 0
+        f = _host(sim, ("pos", "h", "rho", "omega", "acc", "dudt"))
+        gperm = _integer_stages_full(sim, f["pos"], pre["h"], box, fresh=False)
+        vstar = (pre["vel"] + 0.5 * dt * pre["acc"]) + 0.5 * dt * pre["acc"]
+        _slot_sample_parity(sim, gperm, s0, 512, f["pos"], vstar, pre["u"], pre["h"], w.mass, box, p, f,
+                            closure(f["pos"], pre["h"]))
     sim.close()
 
 
