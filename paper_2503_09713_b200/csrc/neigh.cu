@@ -43,8 +43,9 @@ constexpr int kStackSlack = 192;         // above kStackCap - kStackSlack the wa
 constexpr int kPendCap = 64;             // candidate buckets buffered before stage 2 runs
 constexpr int kHitCap = 112;             // buffered hits per lane
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
-constexpr int kHitStride = kHitCap + kHitSlack + 4;   // in u16: 296 B per lane row (8-byte aligned: copied out as u64)
-static_assert(kHitStride % 4 == 0, "hit rows are copied as u64 words");
+constexpr int kHitStride = kHitCap + kHitSlack + 8;   // in u16: 304 B per lane row, 16-byte aligned (copied out as uint4; 76 words
+                                                      // per row also spreads the 32 rows' LDS.128 over all banks)
+static_assert(kHitStride % 8 == 0, "hit rows are copied as 16-byte words");
 constexpr int kShare = 4;               // consecutive groups that share one tree walk
 constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
 constexpr int kSpillCap = 512;            // hits per lane that can spill from the shared-memory row to the warp's global scratch
@@ -67,8 +68,7 @@ struct TravWarpSmem {
                                               // scaled fp32 coordinates relative to the group's centre, r = cutoff^2
     uint32_t cslotb[kGroup];                  // their sorted slots (exact path)
     uint32_t ub[kUbCap];                      // bucket nodes within reach of the kShare groups' common box
-    uint32_t rowoff[kGroup + 4];              // copy-out: first u64 word of each particle's list in the group's block
-    uint16_t hits[32 * kHitStride];
+    __align__(16) uint16_t hits[32 * kHitStride];
 };
 
 struct TravOut {
@@ -126,7 +126,7 @@ struct GroupCtx {
     bool anywrap;         // warp-uniform: some bucket of this group may wrap around a periodic axis
     // fp32 fast path (warp-uniform unless marked): coordinates relative to (cx, cy, cz), scaled by sc (a power of two)
     bool use32;
-    double cx, cy, cz, sc;
+    double cx, cy, cz, sc, ksc;   // ksc = R_kern chi sc
     float ax, ay, az, ra2, rca;   // per lane: scaled relative position, cutoff^2 and cutoff (rounded up) of the query
     float ex, ey, ez;             // scaled half extents of the group's box, rounded up
     float twoA, rcg, rc2g_f;      // 2 max(ex, ey, ez); scaled reach of the group (rounded up) and its square
@@ -184,8 +184,9 @@ __device__ __forceinline__ void record_hit(GroupCtx& G, uint32_t& wp, uint32_t l
 // buckets that may wrap) are exact to 2^-53 |r| in fp64 and are rounded once to fp32: |fl(r) - r| <= 2^-24 |r|. With
 // |r_a| <= A (half extent of the group's box) and |r_b| <= A + 3.01 rcm + 6 E for every candidate that passed the
 // prefilter below, each difference d_k = fl(r_a,k - r_b,k) has |d_k - true| <= E := 1.3e-7 (2 A + 3.1 rcm) (2^-23 =
-// 1.19e-7), hence |d2_f - d2| <= 2 sqrt(3) E d + 3 E^2 + 3.01 2^-24 d2, the thresholds carry 2^-24 relative each, and
-// for every test of a bucket  |v_f - v| <= B/4,  B := E (14 rcm' + 12 E) + 2e-6 rcm'^2,  v = d2 - max(cutoff^2),
+// 1.19e-7), hence |d2_f - d2| <= 2 sqrt(3) E d + 3 E^2 + 3.01 2^-24 d2, the thresholds carry 2^-24 (query) and 3 2^-24
+// (candidate: (float)(R chi h s) squared) relative, and
+// for every test of a bucket  |v_f - v| <= B/4,  B := E (14 rcm' + 12 E) + 2.5e-6 rcm'^2,  v = d2 - max(cutoff^2),
 // rcm' = the larger of the query's and the bucket's reach (true hit: d <= rcm'; true miss: d2 - err(d) is increasing in
 // d beyond rcm', or E > rcm' / sqrt(3) and 12 E^2 covers it). So |v_f| > B implies sign(v_f) = sign(v), and sign(v) is
 // the fp64 decision because that differs from the real-number one only within 1e-15 relative of the cutoff.
@@ -194,7 +195,8 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const TravBox& tb, double rk_chi) {
-    const uint32_t row = lane * kHitStride;
+    const uint32_t rowbase = (uint32_t)__cvta_generic_to_shared(&s.hits[lane * kHitStride]);
+    uint32_t wp = rowbase + 2u * G.wpos;          // 32-bit shared-memory address of the lane's next free entry
     const unsigned long long ax2 = pk2(G.ax, G.ax), ay2 = pk2(G.ay, G.ay), az2 = pk2(G.az, G.az), ra22 = pk2(G.ra2, G.ra2);
     // software pipeline: the next bucket's candidate (one per lane) is in flight while this one is tested
     double px = 0.0, py = 0.0, pz = 0.0, ph = 0.0;
@@ -207,9 +209,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
         const uint32_t blo = plo & ~kWrapBit;
         const bool wrap = (plo & kWrapBit) != 0u;
         G.anywrap |= wrap;
-        const double cx = px, cy = py, cz = pz;
-        const double rc = __dmul_rn(rk_chi, ph);
-        const double rc2 = __dmul_rn(rc, rc);
+        const double cx = px, cy = py, cz = pz, ch = ph;
         if (b + 1 < npend) {
             const uint32_t nlo = s.plo[b + 1] & ~kWrapBit;
             if (lane < s.pn[b + 1]) { px = x[nlo + lane]; py = y[nlo + lane]; pz = z[nlo + lane]; ph = h[nlo + lane]; }
@@ -226,15 +226,18 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                 rz = min_image(rz, tb.L[2], tb.halfL[2], tb.periodic[2]);
             }
             fx = (float)(rx * G.sc); fy = (float)(ry * G.sc); fz = (float)(rz * G.sc);
-            fr = (float)(rc2 * G.sc * G.sc);
+            fr = (float)(ch * G.ksc);                    // scaled cutoff radius, then its square: 3 roundings of 2^-24
+            fr *= fr;
             const float rcn = s.prc[b];
             const float rcm_g = fmaxf(rcn, G.rcg);
             const float E = 1.3e-7f * (G.twoA + 3.1f * rcm_g);
             const float gx = fmaxf(fabsf(fx) - G.ex, 0.f), gy = fmaxf(fabsf(fy) - G.ey, 0.f), gz = fmaxf(fabsf(fz) - G.ez, 0.f);
             keep = keep && (gx * gx + gy * gy + gz * gz <= fmaxf(fr, G.rc2g_f) * 1.0001f + 16.f * E * (rcm_g + E));
             const float rcm = fmaxf(G.rca, rcn);
-            band = E * (14.f * rcm + 12.f * E) + 2e-6f * rcm * rcm;
+            band = E * (14.f * rcm + 12.f * E) + 2.5e-6f * rcm * rcm;
         } else if (keep && !wrap) {   // plain fp64 version (groups too large for the scaled frame); wrapping buckets keep all
+            const double rc = __dmul_rn(rk_chi, ch);
+            const double rc2 = __dmul_rn(rc, rc);
             const double gx = clamp0(dmax(G.gxl - cx, cx - G.gxh));
             const double gy = clamp0(dmax(G.gyl - cy, cy - G.gyh));
             const double gz = clamp0(dmax(G.gzl - cz, cz - G.gzh));
@@ -256,9 +259,8 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             q[0] = 1e18f; q[2] = 1e18f; q[4] = 1e18f; q[6] = 0.f;
         }
         __syncwarp();
-        const uint32_t w0 = (uint32_t)__cvta_generic_to_shared(&s.hits[row + G.wpos]);
+        const uint32_t w0 = wp;
         const uint32_t nhit0 = G.nhit;
-        uint32_t wp = w0;
         bool exact = !G.use32;
         if (G.use32) {
             float amin = 3e38f;
@@ -308,9 +310,8 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             asm volatile("" ::: "memory");
         }
         if (!DIRECT) {
-            const uint32_t got = (wp - w0) >> 1;
-            G.nhit += got;
-            G.wpos += got;
+            G.nhit += (wp - w0) >> 1;
+            G.wpos = (wp - rowbase) >> 1;
             // A row has room for one more bucket only up to kHitCap: when some lane is beyond it, every lane moves
             // its row to its part of the warp's global scratch (the list order is kept: spilled part, then the row);
             // when that is full too the group is counted on and walked a second time writing directly.
@@ -331,6 +332,7 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                     G.hard_overflow = true;
                     if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;
                 }
+                wp = rowbase + 2u * G.wpos;
             }
         }
         G.ncs += nk;
@@ -489,6 +491,25 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
     __syncwarp();
 }
 
+// Box and max h of a leaf group: the group is a tree node (or a single leaf), so its tight box and hmax are the record
+// k_aabb_groups wrote for it (the exact min / max of its particles' positions and h): no reduction over the lanes.
+struct GBox { double xl, yl, zl, xh, yh, zh, hm; };
+__device__ __forceinline__ GBox group_box(uint32_t glo, uint32_t nq, const double* __restrict__ x,
+                                          const double* __restrict__ y, const double* __restrict__ z,
+                                          const double* __restrict__ h, const NodeRec* __restrict__ nodes) {
+    GBox b;
+    if (nq == 1u) {
+        b.xl = b.xh = x[glo]; b.yl = b.yh = y[glo]; b.zl = b.zh = z[glo]; b.hm = h[glo];
+    } else {
+        // the node whose range is the whole group: its index is one end of the range
+        const uint32_t root = ((uint32_t)__ldg(&nodes[glo].other) == glo + nq - 1u) ? glo : glo + nq - 1u;
+        const double2* p = reinterpret_cast<const double2*>(nodes + root);
+        const double2 v0 = __ldg(p), v1 = __ldg(p + 1), v2 = __ldg(p + 2), v3 = __ldg(p + 3);
+        b.xl = v0.x; b.yl = v0.y; b.zl = v1.x; b.xh = v1.y; b.yh = v2.x; b.zh = v2.y; b.hm = v3.x;
+    }
+    return b;
+}
+
 __device__ __forceinline__ uint32_t warp_sum_u32(uint32_t v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -532,15 +553,12 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             double vmax = 0.0, vmin = 1e300;
             for (uint32_t g = g0; g < g0 + ng; ++g) {
                 const uint32_t glo = grp_lo[g], nq = grp_lo[g + 1] - glo;
-                const uint32_t a = glo + (lane < nq ? lane : 0u);
-                const double xi = x[a], yi = y[a], zi = z[a], hi = h[a];
-                const double xl = warp_min(xi), xh = warp_max(xi), yl = warp_min(yi), yh = warp_max(yi);
-                const double zl = warp_min(zi), zh = warp_max(zi), hm = warp_max(hi);
-                const double rr = 2.0 * rk_chi * hm;
-                const double vg = (xh - xl + rr) * (yh - yl + rr) * (zh - zl + rr);
+                const GBox gb = group_box(glo, nq, x, y, z, h, nodes);
+                const double rr = 2.0 * rk_chi * gb.hm;
+                const double vg = (gb.xh - gb.xl + rr) * (gb.yh - gb.yl + rr) * (gb.zh - gb.zl + rr);
                 vmax = dmax(vmax, vg); vmin = dmin(vmin, vg);
-                U.gxl = dmin(U.gxl, xl); U.gxh = dmax(U.gxh, xh); U.gyl = dmin(U.gyl, yl); U.gyh = dmax(U.gyh, yh);
-                U.gzl = dmin(U.gzl, zl); U.gzh = dmax(U.gzh, zh); U.ghm = dmax(U.ghm, hm);
+                U.gxl = dmin(U.gxl, gb.xl); U.gxh = dmax(U.gxh, gb.xh); U.gyl = dmin(U.gyl, gb.yl); U.gyh = dmax(U.gyh, gb.yh);
+                U.gzl = dmin(U.gzl, gb.zl); U.gzh = dmax(U.gzh, gb.zh); U.ghm = dmax(U.ghm, gb.hm);
             }
             const double rr = 2.0 * rk_chi * U.ghm;
             const double vu = (U.gxh - U.gxl + rr) * (U.gyh - U.gyl + rr) * (U.gzh - U.gzl + rr);
@@ -560,9 +578,10 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             const double rc = __dmul_rn(rk_chi, hq);
             G.rc2q = __dmul_rn(rc, rc);
         }
-        // group box and max h (lanes beyond nq replicate lane 0)
-        G.gxl = warp_min(G.xq); G.gxh = warp_max(G.xq); G.gyl = warp_min(G.yq); G.gyh = warp_max(G.yq);
-        G.gzl = warp_min(G.zq); G.gzh = warp_max(G.zq); G.ghm = warp_max(hq);
+        {   // group box and max h
+            const GBox gb = group_box(glo, nq, x, y, z, h, nodes);
+            G.gxl = gb.xl; G.gxh = gb.xh; G.gyl = gb.yl; G.gyh = gb.yh; G.gzl = gb.zl; G.gzh = gb.zh; G.ghm = gb.hm;
+        }
         {
             const double rcg = __dmul_rn(rk_chi, G.ghm);
             G.rc2g = __dmul_rn(rcg, rcg);
@@ -583,6 +602,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                       (!tb.periodic[0] || hx + reach_max < tb.halfL[0]) && (!tb.periodic[1] || hy + reach_max < tb.halfL[1]) &&
                       (!tb.periodic[2] || hz + reach_max < tb.halfL[2]);
             if (!G.use32) G.sc = 1.0;
+            G.ksc = rk_chi * G.sc;
             G.ex = (float)(hx * G.sc) * 1.000001f; G.ey = (float)(hy * G.sc) * 1.000001f; G.ez = (float)(hz * G.sc) * 1.000001f;
             G.twoA = 2.f * fmaxf(G.ex, fmaxf(G.ey, G.ez));
             G.rcg = (float)(rcg * G.sc) * 1.000001f;
@@ -598,9 +618,9 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         if (nu >= 0) refine<false>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
         else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
-        // ---- allocate from the exact counts: lists (block padded to 8 entries = 16 B) and candidate slots ----
-        // every particle's list starts at a multiple of four entries (8 B), so that rows are copied out as u64
-        const uint32_t nhit = qv ? G.nhit : 0u, nhit4 = (nhit + 3u) & ~3u;
+        // ---- allocate from the exact counts: lists and candidate slots ----
+        // every particle's list starts at a multiple of eight entries (16 B), so that rows are copied out as uint4
+        const uint32_t nhit = qv ? G.nhit : 0u, nhit4 = (nhit + 7u) & ~7u;
         const uint32_t nc = G.ncs, nc4 = (nc + 3u) & ~3u;
         uint32_t incl = nhit4;
 #pragma unroll
@@ -642,23 +662,17 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                 // lists: the warp copies one particle's buffered list at a time (coalesced)
                 const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
                 if (!spilled) {
-                    // every list starts at a multiple of four entries of the group's block, so rows leave as u64
-                    // words (the up to three entries of padding are never read); the word offsets go through shared
-                    // memory so that the row loop needs no shuffles
-                    s.rowoff[lane] = (incl - nhit4) >> 2;
-                    if (lane == 31u) s.rowoff[32] = total >> 2;
-                    __syncwarp();
-                    uint64_t* const dst = reinterpret_cast<uint64_t*>(out.lists + lbase);
-                    const uint64_t* const src = reinterpret_cast<const uint64_t*>(s.hits);
-#pragma unroll 4
-                    for (uint32_t p = 0; p < nq; ++p) {
-                        const uint32_t o0 = s.rowoff[p], nw = s.rowoff[p + 1] - o0;
-                        for (uint32_t k = lane; k < nw; k += 32) dst[o0 + k] = src[p * (kHitStride / 4) + k];
-                    }
+                    // every lane copies its own row, 16 bytes per store (the up to seven entries of padding are never
+                    // read): a store instruction touches 32 lists, half a sector each, and consecutive instructions
+                    // fill the sectors in L2; a row-by-row copy by the whole warp is coalesced but costs 30 times the
+                    // instructions
+                    const uint4* src = reinterpret_cast<const uint4*>(&s.hits[lane * kHitStride]);
+                    uint4* dst = reinterpret_cast<uint4*>(out.lists + my_start);
+                    for (uint32_t k = 0; k < (nhit4 >> 3); ++k) dst[k] = src[k];
                 } else {
                     for (uint32_t p = 0; p < nq; ++p) {
                         const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
-                        uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 3u) & ~3u));
+                        uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 7u) & ~7u));
                         const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p);
                         const uint16_t* src = hit_row + (size_t)p * kSpillCap;
                         for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
