@@ -34,10 +34,11 @@ FLOP_PER_PAIR_DENSITY_SWEEP = 16      # q, f, f', two accumulations (per pair pe
 FLOP_PER_PAIR_FORCE = 93              # Eq. 3-6, 8-10 per pair
 FLOP_PER_PAIR_TEST = 13               # exact object-object test per found pair (single pass)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
-# workload (profiles/r1_ncu_all_v22.md); only quoted when bench runs that workload
 KERNEL_NAMES = ("M4", "M5", "M6", "Wendland C2", "Wendland C4", "Wendland C6")   # FLOP_PER_PAIR_* below are the M4 counts
-NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.53e9, "traverse": 4.61e9, "density": 4.95e9}   # profiles/r1_ncu_all_v29.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the committed ncu --set full capture of this
+# workload: NOT measured by this run (bench.py never runs under a profiler); only quoted when bench runs that workload
+NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_all.md"
+NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.53e9, "traverse": 4.61e9, "density": 4.95e9}
 
 
 def reduce_over_ranks(ms_local: float, n_local: float, world: int, device):
@@ -107,6 +108,27 @@ class ClockSampler(threading.Thread):
                 "reasons": [k for k, b in bits.items() if seen & b]}
 
 
+def host_cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_c0_rate():
+    """BASELINE config 0 in full on the oracle: one tree build + density iteration + force evaluation of 16^3 particles."""
+    import oracle as O
+    from paper_2503_09713_b200 import workloads as W
+    w = W.config(0)
+    t0 = time.perf_counter()
+    O.State(w, "grid")
+    dt = time.perf_counter() - t0
+    return w.n / dt, dt
+
+
 def oracle_step_rate(n_side: int, steps: int, warmup: int):
     """Time the oracle (as it stands, 1 thread) on the C2 recipe at n_side^3 particles."""
     import oracle as O
@@ -135,9 +157,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": make_workload(args.workload).name if False else f"{args.workload} (oracle sample {n_side}^3)",
-                       "n_particles": n, "l2": "n/a (CPU)"},
-            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": {"workload": f"{args.workload} (oracle sample {n_side}^3)", "n_particles": n, "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                             "host_cpu": host_cpu_model()},
             "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -187,7 +209,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--ref-side", type=int, default=40, help="lattice side of the oracle's bounded sample")
+    ap.add_argument("--ref-side", type=int, default=40, help="lattice side of the oracle's bounded sample (--impl reference)")
+    ap.add_argument("--cpu-side", type=int, default=64, help="lattice side of the cpu_baseline leg (64 = the smallest point of BASELINE config 4)")
     ap.add_argument("--group-max", type=int, default=0,
                     help="particles per leaf group / bucket, 1..32 (0 = the default 32): the particles-per-leaf sweep of PAPER.md:382")
     ap.add_argument("--morton-bits", type=int, default=0, help="21 (default) or 10: the paper's 30-bit Morton codes (PAPER.md:582, 378)")
@@ -286,12 +309,13 @@ def main():
         fp64_peak = B.measure_fp64_peak()      # TFLOP/s, DFMA microbenchmark run now on this GPU
         K = args.steps
         pairs = st["n_neighbours"]             # pairs in the cache of the last step (self included)
-        sweeps = max(st["h_iter_max"], 1) + 1  # upper bound on Newton sweeps + the Omega pass
+        # Newton sweeps + the closing pass at the converged h, counted on the device by k_density: mean per particle
+        sweeps = st["density_sweeps"] / n if st.get("density_sweeps", 0) > 0 else max(st["h_iter_max"], 1) + 1
         per_stage = {k[3:]: st[k] / K for k in st if k.startswith("ms_") and k != "ms_total"}
         flops = {"density": pairs * (FLOP_PER_PAIR_DENSITY_GATHER + FLOP_PER_PAIR_DENSITY_SWEEP * sweeps),
                  "forces": pairs * FLOP_PER_PAIR_FORCE,
                  "traverse": pairs * FLOP_PER_PAIR_TEST}
-        bytes_ = {"keys": 36 * n, "sort": (8 + 24 * st.get("sort_passes", 8)) * n, "permute": 216 * n, "tree": 60 * n, "aabb": 148 * n,
+        bytes_ = {"keys": 36 * n, "sort": (8 + 24 * st.get("sort_passes", 8)) * n, "permute": 220 * n, "tree": 60 * n, "aabb": 148 * n,
                   "scan": 12 * n, "leapfrog": 272 * n}
         kernels = {}
         per_stage = {k: v for k, v in per_stage.items() if v > 0.0}
@@ -307,17 +331,26 @@ def main():
         traffic = NCU_TRAFFIC_BYTES_CUBE256.get(dom) if (args.workload == "cube256" and not args.sph_kernel and not args.hfact
                                                           and args.group_max in (0, 32)) else None
         roofline.update({"kernel": dom, "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
+                         "traffic_source": f"{NCU_TRAFFIC_SOURCE} (committed ncu capture of this kernel), not measured by this run" if traffic else None,
+                         "peak_note": "hbm peak is the measured copy bandwidth of MEASURED_PEAKS.json, so an hbm frac can read slightly above 1 (nominal 7.7 TB/s)",
                          "peak_source": "sph_measure_fp64_peak DFMA microbenchmark, this run" if dom in flops else hbm_src,
                          "share_of_step": per_stage[dom] / sum(per_stage.values())})
         cpu = None
         if not args.no_cpu_baseline:
-            rate, s_per_step, n_s, t_init = oracle_step_rate(40, 1, 0)
-            cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                   "sample": f"C2 recipe at 40^3 = {n_s} particles, 1 full oracle leapfrog step ({s_per_step:.1f} s) after its white step ({t_init:.1f} s)"}
+            # BASELINE configs on the oracle: config 0 in full (one evaluation of 16^3 particles) and the 64^3 point
+            # of config 4 (the C2 recipe), one full leapfrog step after its white step: ~45 s of CPU work in all
+            c0_rate, c0_s = oracle_c0_rate()
+            rate, s_per_step, n_s, t_init = oracle_step_rate(args.cpu_side, 1, 0)
+            cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "host_cpu": host_cpu_model(),
+                   "sample": f"BASELINE config 4 point {args.cpu_side}^3 = {n_s} particles (the C2 recipe), 1 full oracle leapfrog step "
+                             f"({s_per_step:.1f} s) after its white step ({t_init:.1f} s)",
+                   "config0": {"value": c0_rate, "unit": "particles/s per evaluation (build + density + forces)",
+                               "seconds": c0_s, "sample": "BASELINE config 0 in full: 16^3 particles, one evaluation"}}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": KERNEL_NAMES[args.sph_kernel], "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21,
+                           "density_sweeps_mean": sweeps,
                            "hfact": w.hfact, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "inputs (~0.8 kB/particle resident) larger than the 126 MB L2; no flush",
                            "restarts_last_step": st["restarts"], "h_iter_max": st["h_iter_max"]},

@@ -132,6 +132,19 @@ def sort_keys(key):
     return skey, perm
 
 
+def leaf_reduction(skey, n_red: int):
+    """Alg. 1 on sorted Morton codes: (xi mask u8[N], leaf codes u64[n_leaf], id map u32[n_leaf + 1])."""
+    skey = np.ascontiguousarray(skey, dtype=np.uint64)
+    n = skey.shape[0]
+    xi = np.zeros(n, dtype=np.uint8)
+    lib().orc_leaf_reduction(C.c_int64(n), _p(skey, np.uint64), C.c_int32(int(n_red)), _p(xi, np.uint8))
+    codes = np.zeros(n, dtype=np.uint64)
+    ids = np.zeros(n + 1, dtype=np.uint32)
+    lib().orc_leaf_compact.restype = C.c_int64
+    nl = lib().orc_leaf_compact(C.c_int64(n), _p(skey, np.uint64), _p(xi, np.uint8), _p(codes, np.uint64), _p(ids, np.uint32))
+    return xi, codes[:nl].copy(), ids[:nl + 1].copy()
+
+
 def tree(skey):
     """Radix-tree tables over sorted keys: dict(left, right, lflag, rflag, parent[2N-1], rlo, rhi)."""
     skey = np.ascontiguousarray(skey, dtype=np.uint64)

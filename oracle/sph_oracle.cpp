@@ -292,6 +292,45 @@ void orc_sort(int64_t N, const uint64_t* key, uint32_t* perm, uint64_t* sorted_k
     for (int64_t i = 0; i < N; ++i) { perm[i] = p[i]; sorted_key[i] = key[p[i]]; }
 }
 
+// ---- Alg. 1 (App. C1-C2): removal mask xi over the SORTED Morton codes.
+// Lines 1-5: xi_i = (i == 0) or (m_i != m_{i-1}) (duplicates removed). Lines 6-22, n_red times: for every i,
+// i_-1 and i_-2 are the two kept indices before i, i_+1 the kept index after it; with delta_0 = delta(mu_i, mu_i+1),
+// delta_-1 = delta(mu_i-1, mu_i), delta_-2 = delta(mu_i-2, mu_i-1), the code stays kept unless
+// delta_0 < delta_-1 and delta_-2 < delta_-1 (it is then the second leaf of a two-leaf parent).
+// Readings (A17): "for i in parallel" is taken as a synchronous pass -- every i reads the mask as it was when
+// the pass began; a neighbour that does not exist (i_-1, i_-2 < 0 or i_+1 >= n) gives delta = -1, Karras' convention
+// for out-of-range indices; delta is the common-prefix length of the full 64-bit words (Eq. B2).
+void orc_leaf_reduction(int64_t N, const uint64_t* skey, int32_t n_red, uint8_t* xi) {
+    for (int64_t i = 0; i < N; ++i) xi[i] = (i == 0) || (skey[i] != skey[i - 1]);        // l.1-5
+    std::vector<uint8_t> old(N);
+    for (int32_t pass = 0; pass < n_red; ++pass) {                                         // l.6
+        std::memcpy(old.data(), xi, (size_t)N);
+        for (int64_t i = 0; i < N; ++i) {                                                  // l.7
+            int64_t im1 = i - 1;                                                           // l.8-10
+            while (im1 >= 0 && !old[im1]) --im1;
+            int64_t im2 = im1 - 1;                                                         // l.11-13
+            while (im2 >= 0 && !old[im2]) --im2;
+            int64_t ip1 = i + 1;                                                           // l.14-16
+            while (ip1 < N && !old[ip1]) ++ip1;
+            const int d0 = (ip1 < N) ? clz64(skey[i] ^ skey[ip1]) : -1;                    // l.17
+            const int dm1 = (im1 >= 0) ? clz64(skey[im1] ^ skey[i]) : -1;                  // l.18
+            const int dm2 = (im2 >= 0) ? clz64(skey[im2] ^ skey[im1]) : -1;                // l.19
+            xi[i] = (!(d0 < dm1 && dm2 < dm1)) && old[i];                                  // l.20-22
+        }
+    }
+}
+
+// Stream compaction of the kept codes (Fig. D2): leaf codes mu_leaf and the index map id (the index
+// of every kept code before compaction, closed by id[n_leaf] = N): leaf j holds the sorted objects [id_j, id_j+1)
+// (Alg. 2). Returns n_leaf.
+int64_t orc_leaf_compact(int64_t N, const uint64_t* skey, const uint8_t* xi, uint64_t* leaf_code, uint32_t* id_map) {
+    int64_t n = 0;
+    for (int64_t i = 0; i < N; ++i)
+        if (xi[i]) { leaf_code[n] = skey[i]; id_map[n] = (uint32_t)i; ++n; }
+    id_map[n] = (uint32_t)N;
+    return n;
+}
+
 // ---- O3: radix tree tables (Table B2). Arrays of N-1 internal nodes; parent has 2N-1.
 void orc_tree(int64_t N, const uint64_t* skey, int32_t* left, int32_t* right, uint8_t* lflag, uint8_t* rflag,
               int32_t* parent, int32_t* rlo, int32_t* rhi) {

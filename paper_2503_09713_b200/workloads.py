@@ -1,4 +1,6 @@
-"""Seeded synthetic workload generators (inputs only; none of the method's arithmetic lives here).
+"""Seeded synthetic workload generators (inputs only; none of the method's arithmetic lives here, with one
+stated exception: ``sedov`` shapes its injected-energy profile with the textbook M4 polynomial, "smoothed
+by the kernel" -- an input profile, compared with nothing; neither side's kernels are used or checked through it).
 
 Shared by the oracle-side tests and the CUDA-side tests/bench. NumPy only: this module imports neither
 ``oracle/`` nor the CUDA binding. Recipes follow SURVEY.md §8(d) / DESIGN.md "Input recipe": they stand in

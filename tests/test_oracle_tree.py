@@ -205,3 +205,68 @@ def test_morton_30bit_variant():
     assert np.unique(skey).size < w.n
     t = O.tree(skey)
     assert np.all(t["rhi"] > t["rlo"])
+
+
+# ---------------------------------------------------------------- Alg. 1: duplicate removal and leaf reduction
+
+def _leaf_gold():
+    rows, extra = {}, {}
+    for line in open(os.path.join(GOLD, "leaf_reduction.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        t = line.split()
+        if t[0] in ("keys", "dupkeys", "dupmask", "dupids"):
+            extra[t[0]] = [int(v) for v in t[1:]]
+        else:
+            vals = [int(v) for v in t[1:]]
+            # kept keys, then the id map: the id map starts at the first 0 after a non-zero entry or is the tail
+            # whose last element is 12; split by length: n kept keys followed by n + 1 ids
+            n = (len(vals) - 1) // 2
+            rows[int(t[0])] = (vals[:n], vals[n:])
+    return rows, extra
+
+
+def test_leaf_reduction_worked_example():
+    """Alg. 1 on the Table B2 key list, every pass worked by hand in tests/golden/leaf_reduction.txt."""
+    rows, extra = _leaf_gold()
+    keys = np.array(extra["keys"], dtype=np.uint64)
+    for n_red, (kept, ids) in rows.items():
+        xi, codes, idmap = O.leaf_reduction(keys, n_red)
+        assert list(codes) == kept and list(idmap) == ids, n_red
+        assert list(np.nonzero(xi)[0]) == ids[:-1]
+    xi, codes, idmap = O.leaf_reduction(np.array(extra["dupkeys"], dtype=np.uint64), 0)
+    assert list(xi) == extra["dupmask"] and list(idmap) == extra["dupids"] and list(codes) == [0, 1, 2, 3]
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_leaf_reduction_merges_exactly_the_two_leaf_parents(seed):
+    """App. C2: a code is removable iff it is the second leaf of a parent whose two children are both
+    leaves. Brute force through the radix tree of the codes kept before each pass (built by the recursive oracle
+    builder, which knows nothing of Alg. 1): the codes a pass removes are exactly the right children of the internal
+    nodes whose two children are leaves; leaves stay contiguous, sorted and non-empty."""
+    rng = np.random.default_rng(seed)
+    keys = np.sort(rng.integers(0, 1 << 20, size=3000, dtype=np.uint64) << np.uint64(43 - 7 * seed))
+    keys[100:110] = keys[100]                                  # duplicates
+    keys = np.sort(keys)
+    prev_codes = np.unique(keys)
+    xi0, codes0, ids0 = O.leaf_reduction(keys, 0)
+    assert np.array_equal(codes0, prev_codes) and np.array_equal(keys[ids0[:-1]], codes0)
+    for n_red in range(1, 8):
+        xi, codes, ids = O.leaf_reduction(keys, n_red)
+        t = O.tree(prev_codes)
+        both = (t["lflag"] == 1) & (t["rflag"] == 1)
+        expect_removed = set(prev_codes[t["right"][both]].tolist()) if prev_codes.size > 1 else set()
+        removed = set(prev_codes.tolist()) - set(codes.tolist())
+        assert removed == expect_removed and len(removed) > 0
+        assert np.array_equal(keys[ids[:-1]], codes) and ids[0] == 0 and ids[-1] == keys.size
+        assert np.all(np.diff(ids.astype(np.int64)) > 0) and np.all(np.diff(codes.astype(np.int64)) > 0)
+        prev_codes = codes
+    # every leaf of the reduced list is a prefix class: its objects share more leading bits with one another than with
+    # either neighbouring leaf (the reduced tree "mirrors the initial one", PAPER.md:975)
+    for j in range(len(codes)):
+        lo, hi = int(ids[j]), int(ids[j + 1]) - 1
+        inner = 64 if lo == hi or keys[lo] == keys[hi] else 64 - int(keys[lo] ^ keys[hi]).bit_length()
+        if lo > 0:
+            assert 64 - int(keys[lo - 1] ^ keys[lo]).bit_length() < inner
+        if hi + 1 < keys.size:
+            assert 64 - int(keys[hi] ^ keys[hi + 1]).bit_length() < inner
