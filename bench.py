@@ -213,6 +213,8 @@ def main():
     ap.add_argument("--cpu-side", type=int, default=64, help="lattice side of the cpu_baseline leg (64 = the smallest point of BASELINE config 4)")
     ap.add_argument("--group-max", type=int, default=0,
                     help="particles per leaf group / bucket, 1..32 (0 = the default 32): the particles-per-leaf sweep of PAPER.md:382")
+    ap.add_argument("--leaf-reduction", type=int, default=0,
+                    help="0 = off (group_max rule); k >= 1: leaf groups from the paper's Alg. 1 with n_red = k - 1 passes (PAPER.md:911-963)")
     ap.add_argument("--morton-bits", type=int, default=0, help="21 (default) or 10: the paper's 30-bit Morton codes (PAPER.md:582, 378)")
     ap.add_argument("--sph-kernel", type=int, default=0, help="0 M4 (default, the BASELINE configs), 1 M5, 2 M6, 3/4/5 Wendland C2/C4/C6")
     ap.add_argument("--hfact", type=float, default=0.0, help="h_fact (default 1.2; the paper uses 1.0 with M6, PAPER.md:208)")
@@ -247,7 +249,7 @@ def main():
         w.h0 = w.h0 * (hf / w.hfact)
         w.kernel, w.hfact = args.sph_kernel, hf
     n = w.n
-    sim = B.Sim.from_workload(w, params=B.params_for(w, group_max=args.group_max, morton_bits=args.morton_bits))   # inputs resident in HBM; includes the white step
+    sim = B.Sim.from_workload(w, params=B.params_for(w, group_max=args.group_max, morton_bits=args.morton_bits, leaf_reduction=args.leaf_reduction))   # inputs resident in HBM; includes the white step
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -349,7 +351,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": KERNEL_NAMES[args.sph_kernel], "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21,
+                "config": {"workload": w.name, "n_particles": n, "neighbours_mean": st["nbr_mean"], "kernel": KERNEL_NAMES[args.sph_kernel], "group_max": args.group_max or 32, "morton_bits": args.morton_bits or 21, "leaf_reduction": args.leaf_reduction, "n_groups": st["n_groups"],
                            "density_sweeps_mean": sweeps,
                            "hfact": w.hfact, "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "inputs (~0.8 kB/particle resident) larger than the 126 MB L2; no flush",

@@ -86,7 +86,11 @@ typedef struct {
                            (SURVEY.md 8(f) item 4): the 30-bit code is kept in the top bits of the
                            64-bit key word (bits 62..33, the low 33 bits zero), sorted with four radix passes, ties
                            (particles of one 2^-10 cell) stay in their previous order; results do not depend on it   */
-  int32_t reserved3;
+  int32_t leaf_reduction; /* 0  (off: leaf groups by the group_max rule). k >= 1: the paper's own leaf construction, Alg. 1
+                           (PAPER.md:911-963): duplicate codes removed, then n_red = k - 1 reduction passes merge
+                           sibling leaves; the leaf groups / traversal buckets are those reduced leaves (a leaf that
+                           holds more than group_max particles is split by the group_max rule). The A/B variant of
+                           SURVEY.md 8(f) item 1; results do not depend on it, the speed does (Fig. 16) */
 } sph_params;
 
 /* Device-memory hooks so that the host framework (PyTorch's caching allocator) owns device memory.
@@ -199,6 +203,11 @@ int sph_get_neighbours(sph_ctx* ctx, sph_mem mem, uint64_t* offs, uint32_t* idx,
  * SPH_ERR_ARG if the range leaves [0, N); SPH_ERR_CAP if cap < offs[count] - offs[0]. */
 int sph_get_neighbours_range(sph_ctx* ctx, sph_mem mem, int64_t first, int64_t count, uint64_t* offs, uint32_t* idx,
                              uint64_t cap);
+/* Reduced leaves of Alg. 1 (only with sph_params.leaf_reduction >= 1; SPH_ERR_ORDER otherwise): *n_leaves, their
+ * Morton codes leaf_codes[n_leaves] and the index map id_map[n_leaves + 1] (sorted slot of each kept code, closed by
+ * N; leaf j holds the sorted slots [id_map[j], id_map[j+1]), Alg. 2). Buffers must hold N and N + 1
+ * entries; either may be NULL. */
+int sph_get_leaves(sph_ctx* ctx, sph_mem mem, int64_t* n_leaves, uint64_t* leaf_codes, uint32_t* id_map);
 int sph_get_stats(sph_ctx* ctx, sph_stats* out);
 int sph_reset_timers(sph_ctx* ctx);
 const char* sph_last_error(const sph_ctx* ctx);

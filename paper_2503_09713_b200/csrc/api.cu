@@ -268,6 +268,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     if (c->p.morton_bits == 0) c->p.morton_bits = 21;
     if (c->p.morton_bits != 21 && c->p.morton_bits != 10) return fail(c, SPH_ERR_ARG, "morton_bits must be 21 or 10 (0 = default 21)");
     if (c->p.group_max < 1 || c->p.group_max > kGroup) return fail(c, SPH_ERR_ARG, "group_max must be in 1..32 (0 = default 32)");
+    if (c->p.leaf_reduction < 0 || c->p.leaf_reduction > 64) return fail(c, SPH_ERR_ARG, "leaf_reduction must be in 0..64");
     if (!(c->p.hfact > 0) || !(c->p.chi >= 1.0) || !(c->p.lambda > 1.0) || !(c->p.eps_h > 0) || c->p.max_h_iter < 1)
         return fail(c, SPH_ERR_ARG, "bad parameters");
     c->stream = (cudaStream_t)cuda_stream;
@@ -293,6 +294,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->parent, 2 * n));
     SPH_TRY(dalloc(c, &c->visit, n));
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
+    if (c->p.leaf_reduction >= 1) { SPH_TRY(dalloc(c, &c->xi_a, n)); SPH_TRY(dalloc(c, &c->xi_b, n)); SPH_TRY(dalloc(c, &c->lscan, n + 1)); }
     SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
     SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
     SPH_TRY(dalloc(c, &c->trav_hit_scratch, trav_hit_scratch_entries()));
@@ -606,6 +608,33 @@ int sph_get_neighbours_range(sph_ctx* c, sph_mem mem, int64_t first, int64_t cou
 int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
     SPH_TRY(check_ctx(c));
     return sph_get_neighbours_range(c, mem, 0, c->N, offs, idx, cap);
+}
+
+int sph_get_leaves(sph_ctx* c, sph_mem mem, int64_t* n_leaves, uint64_t* leaf_codes, uint32_t* id_map) {
+    SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
+    if (c->p.leaf_reduction < 1) return fail(c, SPH_ERR_ORDER, "sph_get_leaves needs sph_params.leaf_reduction >= 1");
+    if (c->state < S_TREE) return fail(c, SPH_ERR_ORDER, "no tree built");
+    const int64_t N = c->N;
+    uint32_t nl = 0;
+    SPH_CUDA(c, cudaMemcpyAsync(&nl, c->lscan + N, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    uint64_t* t_codes = nullptr;
+    uint32_t* t_ids = nullptr;
+    uint64_t* codes = leaf_codes;
+    uint32_t* ids = id_map;
+    if (mem == SPH_MEM_HOST) {
+        if (leaf_codes) { SPH_TRY(dalloc(c, &t_codes, (size_t)N)); codes = t_codes; }
+        if (id_map) { SPH_TRY(dalloc(c, &t_ids, (size_t)N + 1)); ids = t_ids; }
+    }
+    int rc = launch_leaf_export(c, codes, ids);
+    cudaStreamSynchronize(c->stream);
+    if (rc == SPH_OK && t_codes) rc = copy_raw(c, mem, leaf_codes, t_codes, (size_t)nl * sizeof(uint64_t));
+    if (rc == SPH_OK && t_ids) rc = copy_raw(c, mem, id_map, t_ids, ((size_t)nl + 1) * sizeof(uint32_t));
+    cudaStreamSynchronize(c->stream);
+    if (t_codes) dfree(c, t_codes);
+    if (t_ids) dfree(c, t_ids);
+    if (n_leaves) *n_leaves = (int64_t)nl;
+    return rc;
 }
 
 int sph_reset_timers(sph_ctx* c) {

@@ -118,6 +118,10 @@ struct sph_ctx {
     uint32_t* gflag = nullptr;          // N   1 at the first slot of each leaf group
     uint32_t* gscan = nullptr;          // N+1 exclusive scan of gflag (u32)
     uint32_t* grp_lo = nullptr;         // Ng+1 first slot of group g (grp_lo[Ng] = N)
+    // Alg. 1 variant (sph_params.leaf_reduction >= 1): removal mask (two buffers, the passes alternate) and its
+    // exclusive scan = leaf id of every sorted slot (+1 from the slot's own flag)
+    uint32_t *xi_a = nullptr, *xi_b = nullptr, *lscan = nullptr;
+    uint32_t* xi_final = nullptr;       // the buffer holding the final mask of the last build
     int64_t n_groups = 0;
     // neighbour cache, group-local (a4): per group a candidate array (sorted slots of the particles
     // that passed the traversal's prefilter) and per particle an ascending list of 16-bit indices into it
@@ -188,6 +192,7 @@ int launch_keys(sph_ctx* c);                                   // keys.cu
 int launch_sort(sph_ctx* c);                                   // sort.cu   (key,val) -> sorted into key,val
 int launch_permute(sph_ctx* c);                                // permute.cu
 int launch_tree(sph_ctx* c);                                   // tree.cu   karras + groups
+int launch_leaf_export(sph_ctx* c, uint64_t* codes, uint32_t* ids);   // tree.cu   Alg. 1 leaves -> codes + id map
 int launch_aabb(sph_ctx* c);                                   // tree.cu
 int launch_traverse(sph_ctx* c);                               // neigh.cu  single pass: walk, test, write cache
 int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out, int64_t first, int64_t count);   // neigh.cu  group-local lists -> CSR (getter)

@@ -58,6 +58,8 @@ struct TravBox {
     int periodic[3];
     double gg_pad;                       // absolute slack added to the conservative box test
     uint32_t gmax;                       // nodes with <= gmax particles are buckets (sph_params.group_max)
+    const uint32_t* lscan;               // Alg. 1 variant (else null): scan of the removal mask; a bucket must also lie
+                                         // inside one reduced leaf: lscan[hi + 1] == lscan[lo + 1]
 };
 
 struct TravWarpSmem {
@@ -366,6 +368,7 @@ __device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, cons
         r.rlo = min(e, (uint32_t)other);
         r.rhi = max(e, (uint32_t)other);
         r.small = (r.rhi - r.rlo + 1) <= tb.gmax;
+        if (tb.lscan && r.small) r.small = __ldg(tb.lscan + r.rhi + 1) == __ldg(tb.lscan + r.rlo + 1);
     }
     r.prc = (float)(rk_chi * bhm * G.sc) * 1.000001f;   // the node's reach in the group's scaled units, rounded up
     const double ext = rk_chi * dmax(G.ghm, bhm) * (1.0 + 1e-9) + tb.gg_pad;
@@ -730,6 +733,7 @@ int launch_traverse(sph_ctx* c) {
     }
     tb.gg_pad = 1e-14 * Lmax;
     tb.gmax = (uint32_t)c->p.group_max;
+    tb.lscan = c->p.leaf_reduction >= 1 ? c->lscan : nullptr;
     const double rk_chi = kern_radius(c->p.kernel) * c->p.chi;
     TravOut out;
     out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;

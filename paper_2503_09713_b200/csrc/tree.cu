@@ -15,10 +15,48 @@ __device__ __forceinline__ int delta_aug(const uint64_t* __restrict__ key, int N
     return 64 + __clz(i ^ j);
 }
 
+// ---- Alg. 1: removal mask over the sorted codes. Lines 1-5: duplicates; lines 6-22: one
+// reduction pass (every thread reads the mask of the previous pass: a synchronous pass, reading A17).
+// delta = common-prefix length of the code words (Eq. B2), -1 for a neighbour that does not exist.
+__global__ void __launch_bounds__(256) k_leaf_mask_init(int64_t N, const uint64_t* __restrict__ key, uint32_t* __restrict__ xi) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) xi[i] = (i == 0 || key[i] != key[i - 1]) ? 1u : 0u;
+}
+__global__ void __launch_bounds__(256) k_leaf_reduce_pass(int64_t N, const uint64_t* __restrict__ key,
+                                                          const uint32_t* __restrict__ xin, uint32_t* __restrict__ xout) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    if (!xin[i]) { xout[i] = 0u; return; }
+    int64_t im1 = i - 1;
+    while (im1 >= 0 && !xin[im1]) --im1;
+    int64_t im2 = im1 - 1;
+    while (im2 >= 0 && !xin[im2]) --im2;
+    int64_t ip1 = i + 1;
+    while (ip1 < N && !xin[ip1]) ++ip1;
+    const uint64_t ki = key[i];
+    const int d0 = (ip1 < N) ? __clzll((long long)(ki ^ key[ip1])) : -1;
+    const int dm1 = (im1 >= 0) ? __clzll((long long)(key[im1] ^ ki)) : -1;
+    const int dm2 = (im2 >= 0) ? __clzll((long long)(key[im2] ^ key[im1])) : -1;
+    xout[i] = (d0 < dm1 && dm2 < dm1) ? 0u : 1u;     // second leaf of a two-leaf parent: removed
+}
+// kept codes and their index map by the scan of the mask (stream compaction)
+__global__ void __launch_bounds__(256) k_leaf_export(int64_t N, const uint64_t* __restrict__ key, const uint32_t* __restrict__ xi,
+                                                     const uint32_t* __restrict__ lscan, uint64_t* codes, uint32_t* ids) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    if (xi[i]) {
+        if (codes) codes[lscan[i]] = key[i];
+        if (ids) ids[lscan[i]] = (uint32_t)i;
+    }
+    if (i == N - 1 && ids) ids[lscan[N]] = (uint32_t)N;
+}
+
 // one thread per internal node i in [0, N-2]
+// lscan (may be null): exclusive scan of the Alg. 1 mask; the slots lo..hi lie in one reduced leaf iff no code is kept
+// in (lo, hi], i.e. lscan[hi + 1] == lscan[lo + 1]
 __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __restrict__ key, NodeRec* __restrict__ nodes,
                                                 int32_t* __restrict__ parent, uint32_t* __restrict__ gflag, int gmax,
-                                                const DevScalars* __restrict__ sc) {
+                                                const uint32_t* __restrict__ lscan, const DevScalars* __restrict__ sc) {
     if (sc->sort_redo) return;   // keys are not in order (sort.cu: k_sort_repair gave up): no groups, nothing downstream runs
     const int N = (int)N64;
     const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
@@ -46,12 +84,14 @@ __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __r
     parent[(lo == gamma) ? (N - 1 + gamma) : gamma] = (int32_t)i;
     parent[(hi == gamma + 1) ? (N - 1 + gamma + 1) : (gamma + 1)] = (int32_t)i;
     if (i == 0) parent[0] = -1;
-    // leaf groups: children of nodes with more than gmax (sph_params.group_max <= kGroup) particles that themselves hold <= gmax
-    if (hi - lo + 1 <= gmax) {
+    // leaf groups: the maximal nodes that hold <= gmax (sph_params.group_max <= kGroup) particles and, in the Alg. 1
+    // variant, lie inside one reduced leaf: children that qualify of a node that does not
+    auto groupable = [&](int a, int b) { return b - a + 1 <= gmax && (!lscan || lscan[b + 1] == lscan[a + 1]); };
+    if (groupable(lo, hi)) {
         if (i == 0) gflag[0] = 1u;   // the whole tree is one group
     } else {
-        if (gamma - lo + 1 <= gmax) gflag[lo] = 1u;        // left child covers [lo, gamma]
-        if (hi - gamma <= gmax) gflag[gamma + 1] = 1u;     // right child covers [gamma + 1, hi]
+        if (groupable(lo, gamma)) gflag[lo] = 1u;          // left child covers [lo, gamma]
+        if (groupable(gamma + 1, hi)) gflag[gamma + 1] = 1u;   // right child covers [gamma + 1, hi]
     }
 }
 
@@ -198,8 +238,23 @@ __global__ void k_single_group(uint32_t* gflag) { gflag[0] = 1u; }
 int launch_tree(sph_ctx* c) {
     const int64_t N = c->N;
     SPH_CUDA(c, cudaMemsetAsync(c->gflag, 0, (size_t)N * sizeof(uint32_t), c->stream));
+    const uint32_t* lscan = nullptr;
+    if (c->p.leaf_reduction >= 1) {
+        // Alg. 1: duplicate mask, n_red = leaf_reduction - 1 passes, scan (leaf ids)
+        uint32_t *a = c->xi_a, *b = c->xi_b;
+        k_leaf_mask_init<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, a);
+        c->launches++;
+        for (int pass = 1; pass < c->p.leaf_reduction; ++pass) {
+            k_leaf_reduce_pass<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, a, b);
+            c->launches++;
+            uint32_t* t = a; a = b; b = t;
+        }
+        c->xi_final = a;
+        SPH_TRY(launch_scan_u32_u32(c, a, c->lscan, N, nullptr));
+        lscan = c->lscan;
+    }
     if (N >= 2) {
-        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag, c->p.group_max, c->d_sc);
+        k_karras<<<div_up(N - 1, 256), 256, 0, c->stream>>>(N, c->key, c->nodes, c->parent, c->gflag, c->p.group_max, lscan, c->d_sc);
         c->launches++;
     } else {
         k_single_group<<<1, 1, 0, c->stream>>>(c->gflag);
@@ -207,6 +262,13 @@ int launch_tree(sph_ctx* c) {
     }
     SPH_TRY(launch_scan_u32_u32(c, c->gflag, c->gscan, N, nullptr));
     k_group_fill<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->gflag, c->gscan, c->grp_lo, c->d_sc);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int launch_leaf_export(sph_ctx* c, uint64_t* codes, uint32_t* ids) {
+    k_leaf_export<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->key, c->xi_final, c->lscan, codes, ids);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

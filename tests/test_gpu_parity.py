@@ -961,3 +961,51 @@ def test_morton_30bit_variant_stage_and_step_parity(make):
     assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
     _invariants(w, sim)
     sim.close()
+
+
+@pytest.mark.parametrize("k", [1, 2, 4, 6, 9])
+def test_leaf_reduction_variant_is_exact(k):
+    """sph_params.leaf_reduction = k: the paper's own leaf construction (Alg. 1: duplicate removal,
+    n_red = k - 1 reduction passes, compaction) as the A/B variant of the group_max rule. The reduced leaves (codes and
+    index map) are bit-exact against the oracle's Alg. 1; the leaf groups are those leaves (split by the group_max rule
+    where a leaf holds more than 32 particles); every later stage stays in parity, neighbour sets included."""
+    from paper_2503_09713_b200 import binding as B
+    cases = [W.random_cloud(3000, seed=11), W.sod(16, 12), W.cube(16, jitter=0.05, vel_amp=0.02, seed=7)]
+    cases[2].morton_bits = 10                                   # 30-bit codes: whole cells of duplicates
+    cases[0].pos[:, 100:104] = cases[0].pos[:, 100:101]         # coincident particles
+    for w in cases:
+        w.leaf_reduction = k
+        sim = _sim(w)
+        _stage_parity(w, sim)
+        skey = sim.get_keys_perm()[0]
+        codes, ids = sim.get_leaves()
+        xi, ocodes, oids = O.leaf_reduction(skey, k - 1)
+        assert np.array_equal(codes, ocodes) and np.array_equal(ids, oids)
+        st = sim.stats()
+        sizes = np.diff(oids.astype(np.int64))
+        assert st["n_groups"] == len(ocodes) if sizes.max() <= 32 else st["n_groups"] > len(ocodes)
+        sim.step_leapfrog(); sim.step_leapfrog()
+        _invariants(w, sim)
+        codes, ids = sim.get_leaves()
+        xi, ocodes, oids = O.leaf_reduction(sim.get_keys_perm()[0], k - 1)
+        assert np.array_equal(codes, ocodes) and np.array_equal(ids, oids)
+        sim.close()
+
+
+def test_leaf_reduction_variant_sampled_parity_128():
+    """The Alg. 1 variant at 128^3 with n_red = 4 (the paper's optimum, ~10-16 particles per leaf): leaves
+    and integer stages bit-exact on all particles, sets and fields on Morton blocks, shared walks on."""
+    w = W.cube(128, jitter=0.1, steps=2)
+    w.leaf_reduction = 5
+    box, p = O.workload_box_params(w)
+    sim = _sim(w)
+    gperm = _integer_stages_full(sim, w.pos, w.h0, box, fresh=True)
+    codes, ids = sim.get_leaves()
+    xi, ocodes, oids = O.leaf_reduction(sim.get_keys_perm()[0], 4)
+    assert np.array_equal(codes, ocodes) and np.array_equal(ids, oids)
+    assert sim.stats()["n_groups"] == len(ocodes) and np.diff(oids.astype(np.int64)).max() == 16
+    f = _host(sim, ("h", "rho", "omega", "acc", "dudt"))
+    for s0 in (0, 1024 * 777, w.n - 1024):
+        _slot_sample_parity(sim, gperm, s0, 1024, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f)
+    _stepped_parity(w, sim, 2, (2,), (0.0, 0.5))
+    sim.close()
