@@ -38,7 +38,8 @@ class Params(C.Structure):
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("newton_literal", C.c_int32),
                 ("cs0", C.c_double), ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
                 ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
-                ("max_recycle", C.c_int32), ("kernel", C.c_int32)]
+                ("max_recycle", C.c_int32), ("kernel", C.c_int32), ("alpha_min", C.c_double), ("alpha_max", C.c_double),
+                ("sigma_decay", C.c_double), ("av_switch", C.c_int32), ("pad_", C.c_int32)]
 
 
 def make_box(lo, hi, periodic) -> Box:
@@ -47,8 +48,10 @@ def make_box(lo, hi, periodic) -> Box:
 
 def make_params(gamma=5.0 / 3.0, hfact=1.2, chi=1.1, lam=1.2, eps_h=1e-6, alpha_av=1.0, beta_av=2.0, beta_u=1.0,
                 c_cour=0.3, c_force=0.25, max_h_iter=50, max_restarts=50, eos_isothermal=None, point_mass=None,
-                newton_literal=0, eps_v=0.0, lambda_stiff=2.0, max_recycle=10, kernel=0) -> Params:
+                newton_literal=0, eps_v=0.0, lambda_stiff=2.0, max_recycle=10, kernel=0, av_switch=0, alpha_min=0.0,
+                alpha_max=1.0, sigma_decay=0.1) -> Params:
     p = Params()
+    p.av_switch, p.alpha_min, p.alpha_max, p.sigma_decay = int(av_switch), alpha_min, alpha_max, sigma_decay
     p.hfact, p.gamma, p.chi, p.lam, p.eps_h = hfact, gamma, chi, lam, eps_h
     p.alpha_av, p.beta_av, p.beta_u, p.c_cour, p.c_force = alpha_av, beta_av, beta_u, c_cour, c_force
     p.max_h_iter, p.max_restarts, p.newton_literal = max_h_iter, max_restarts, newton_literal
@@ -72,6 +75,8 @@ def workload_box_params(w, **kw):
         kw = dict(dict(eps_v=w.eps_v), **kw)
     if getattr(w, "kernel", 0):
         kw = dict(dict(kernel=w.kernel), **kw)
+    if getattr(w, "av_switch", 0):
+        kw = dict(dict(av_switch=1), **kw)
     return (make_box(w.box_lo, w.box_hi, w.periodic),
             make_params(gamma=w.gamma, hfact=w.hfact, eos_isothermal=w.eos_isothermal, point_mass=w.point_mass, **kw))
 
@@ -97,6 +102,10 @@ def lib():
         _lib.orc_evaluate.restype = C.c_int32
         _lib.orc_step.restype = C.c_int32
         _lib.orc_step2.restype = C.c_int32
+        _lib.orc_step3.restype = C.c_int32
+        _lib.orc_evaluate_alpha.restype = C.c_int32
+        _lib.orc_alpha_update.restype = None
+        _lib.orc_set_alpha.restype = None
     return _lib
 
 
@@ -219,12 +228,36 @@ def h_bisect(pos, m, box: Box, hfact, h_lo, h_hi, kernel=0):
     return out
 
 
-def forces(pos, vel, m, h, rho, omega, u, offs, idx, box: Box, p: Params):
+def alpha_update(pos, vel, acc, m, h, rho, omega, u, offs, idx, box: Box, p: Params, dt, alpha):
+    """G12-G13 with reading A18: dict(alpha, divv, curlv, alpha_loc)."""
+    pos, vel, acc, m, h, rho, omega, u, alpha = (_f64(a) for a in (pos, vel, acc, m, h, rho, omega, u, alpha))
+    n = pos.shape[1]
+    out = dict(alpha=np.empty(n), divv=np.empty(n), curlv=np.empty(n), alpha_loc=np.empty(n))
+    set_kernel(p.kernel)
+    lib().orc_alpha_update(C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(acc, np.float64), _p(m, np.float64),
+                           _p(h, np.float64), _p(rho, np.float64), _p(omega, np.float64), _p(u, np.float64),
+                           _p(offs, np.uint64), _p(idx, np.uint32), C.byref(box), C.byref(p), C.c_double(dt),
+                           _p(alpha, np.float64), _p(out["alpha"], np.float64), _p(out["divv"], np.float64),
+                           _p(out["curlv"], np.float64), _p(out["alpha_loc"], np.float64))
+    return out
+
+
+def forces(pos, vel, m, h, rho, omega, u, offs, idx, box: Box, p: Params, alpha=None):
     pos, vel, m, h, rho, omega, u = (_f64(a) for a in (pos, vel, m, h, rho, omega, u))
     n = pos.shape[1]
     acc = np.empty((3, n))
     dudt = np.empty(n)
     set_kernel(p.kernel)
+    if alpha is not None:
+        alpha = _f64(alpha)
+        lib().orc_set_alpha(_p(alpha, np.float64))
+    try:
+        return _forces_call(pos, vel, m, h, rho, omega, u, offs, idx, box, p, acc, dudt, n)
+    finally:
+        lib().orc_set_alpha(None)
+
+
+def _forces_call(pos, vel, m, h, rho, omega, u, offs, idx, box, p, acc, dudt, n):
     dt = lib().orc_forces(C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(m, np.float64),
                           _p(h, np.float64), _p(rho, np.float64), _p(omega, np.float64), _p(u, np.float64),
                           _p(offs, np.uint64), _p(idx, np.uint32), C.byref(box), C.byref(p), _p(acc, np.float64),
@@ -235,8 +268,9 @@ def forces(pos, vel, m, h, rho, omega, u, offs, idx, box: Box, p: Params):
 _ERR = {-1: "h iteration did not converge within max_h_iter", -2: "more than max_restarts chi-restarts"}
 
 
-def evaluate(pos, vel, m, u, h, box: Box, p: Params, mode="grid"):
-    """Neighbours -> h/rho/Omega with chi-restarts -> forces and dt, for a given state (h = h^n guess)."""
+def evaluate(pos, vel, m, u, h, box: Box, p: Params, mode="grid", alpha=None):
+    """Neighbours -> h/rho/Omega with chi-restarts -> [shock switch] -> forces and dt, for a given state (h = h^n guess).
+    With p.av_switch and `alpha` (the alpha^n array) the result carries the updated alpha (white step: a^n = 0, dt = 0)."""
     pos, vel, m, u = (_f64(a) for a in (pos, vel, m, u))
     h = np.array(h, dtype=np.float64, copy=True)
     n = pos.shape[1]
@@ -244,11 +278,16 @@ def evaluate(pos, vel, m, u, h, box: Box, p: Params, mode="grid"):
     dt = C.c_double()
     nn = C.c_int64()
     set_kernel(p.kernel)
-    rc = lib().orc_evaluate(C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(m, np.float64),
-                            _p(u, np.float64), _p(h, np.float64), C.byref(box), C.byref(p),
-                            C.c_int32(0 if mode == "brute" else 1), _p(out["rho"], np.float64),
-                            _p(out["omega"], np.float64), _p(out["acc"], np.float64), _p(out["dudt"], np.float64),
-                            C.byref(dt), C.byref(nn))
+    args = [C.c_int64(n), _p(pos, np.float64), _p(vel, np.float64), _p(m, np.float64),
+            _p(u, np.float64), _p(h, np.float64), C.byref(box), C.byref(p),
+            C.c_int32(0 if mode == "brute" else 1), _p(out["rho"], np.float64),
+            _p(out["omega"], np.float64), _p(out["acc"], np.float64), _p(out["dudt"], np.float64),
+            C.byref(dt), C.byref(nn)]
+    if alpha is not None:
+        out["alpha"] = np.array(alpha, dtype=np.float64, copy=True)
+        rc = lib().orc_evaluate_alpha(*args, _p(out["alpha"], np.float64))
+    else:
+        rc = lib().orc_evaluate(*args)
     if rc < 0:
         raise RuntimeError("oracle: " + _ERR.get(rc, str(rc)))
     out.update(dt=dt.value, restarts=int(rc), n_neigh=nn.value)
@@ -263,8 +302,11 @@ class State:
         self.mode = mode
         self.pos, self.vel, self.m, self.u = (np.array(a, dtype=np.float64, copy=True)
                                               for a in (w.pos, w.vel, w.mass, w.u))
-        ev = evaluate(self.pos, self.vel, self.m, self.u, w.h0, self.box, self.p, mode)   # "white" step
+        self.alpha = np.full(self.pos.shape[1], self.p.alpha_min) if self.p.av_switch else None
+        ev = evaluate(self.pos, self.vel, self.m, self.u, w.h0, self.box, self.p, mode, alpha=self.alpha)   # "white" step
         self.h, self.rho, self.omega, self.acc, self.dudt = ev["h"], ev["rho"], ev["omega"], ev["acc"], ev["dudt"]
+        if self.alpha is not None:
+            self.alpha = ev["alpha"]
         self.dt = ev["dt"]
         self.restarts = ev["restarts"]
         self.t = 0.0
@@ -277,11 +319,12 @@ class State:
         mult = C.c_double(getattr(self, "cfl_mult", 1.0))
         nrec = C.c_int32()
         set_kernel(self.p.kernel)
-        rc = lib().orc_step2(C.c_int64(n), _p(self.pos, np.float64), _p(self.vel, np.float64), _p(self.m, np.float64),
+        rc = lib().orc_step3(C.c_int64(n), _p(self.pos, np.float64), _p(self.vel, np.float64), _p(self.m, np.float64),
                              _p(self.u, np.float64), _p(self.h, np.float64), _p(self.acc, np.float64),
                              _p(self.dudt, np.float64), C.byref(self.box), C.byref(self.p),
                              C.c_int32(0 if self.mode == "brute" else 1), C.c_double(dt), _p(self.rho, np.float64),
-                             _p(self.omega, np.float64), C.byref(dtn), C.byref(mult), C.byref(nrec))
+                             _p(self.omega, np.float64), C.byref(dtn), C.byref(mult), C.byref(nrec),
+                             _p(self.alpha, np.float64) if getattr(self, "alpha", None) is not None else None)
         if rc < 0:
             raise RuntimeError("oracle: " + _ERR.get(rc, str(rc)))
         self.restarts = int(rc)

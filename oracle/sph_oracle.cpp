@@ -56,6 +56,10 @@ struct orc_params {
     double lambda_stiff; // stiffness of the CFL multiplier G10; value not given, reading A16
     int32_t max_recycle; // cap on corrector re-cycles per step
     int32_t kernel;      // 0 = M4, 1 = M5, 2 = M6, 3-5 = Wendland C2, C4, C6 (informational here: the selector is orc_set_kernel)
+    // shock switch (G11-G13; runscript constants PAPER.md:1412-1415; reading A18)
+    double alpha_min, alpha_max, sigma_decay;
+    int32_t av_switch;   // 0 = constant alpha_av (reading A10); 1 = per-particle alpha_a evolved by G13
+    int32_t pad_;
 };
 
 }  // extern "C"
@@ -301,8 +305,9 @@ void orc_sort(int64_t N, const uint64_t* key, uint32_t* perm, uint64_t* sorted_k
 // the pass began; a neighbour that does not exist (i_-1, i_-2 < 0 or i_+1 >= n) gives delta = -1, Karras' convention
 // for out-of-range indices; delta is the common-prefix length of the full 64-bit words (Eq. B2).
 void orc_leaf_reduction(int64_t N, const uint64_t* skey, int32_t n_red, uint8_t* xi) {
+    if (N < 1) return;
     for (int64_t i = 0; i < N; ++i) xi[i] = (i == 0) || (skey[i] != skey[i - 1]);        // l.1-5
-    std::vector<uint8_t> old(N);
+    std::vector<uint8_t> old((size_t)N);
     for (int32_t pass = 0; pass < n_red; ++pass) {                                         // l.6
         std::memcpy(old.data(), xi, (size_t)N);
         for (int64_t i = 0; i < N; ++i) {                                                  // l.7
@@ -525,6 +530,71 @@ void orc_h_bisect(int64_t N, const double* pos, const double* m, const orc_box* 
     }
 }
 
+// ---- Shock switch (G11-G13). The paper gives the implicit update G13 and the runscript constants
+// (alpha_min = 0, alpha_max = 1, sigma_decay = 0.1) but neither alpha_loc nor tau: it defers to
+// Price et al. (2018) Sect. 2.2.9, which is not in /root/reference. Reading A18 restates that section as far
+// as this build could: with the SPH first-derivative estimate of any field f at particle a,
+//     d_j f |_a = -(1 / (Omega_a rho_a)) sum_b m_b (f_a - f_b) r_hat_j F_ab(h_a),
+//   div v, curl v and the tensor d_j v_i from v* (G12), div a from a^n,
+//   d(div v)/dt = div a - sum_ij (d_j v_i)(d_i v_j),
+//   xi = (div v)^2 / ((div v)^2 + |curl v|^2)   (1 if both vanish),
+//   A = xi max(-d(div v)/dt, 0),  alpha_loc = min(max(10 h^2 A / c_s^2, alpha_min), alpha_max)
+//       (c_s = 0: alpha_max if A > 0, else alpha_min),
+//   tau = h / (sigma_decay c_s)   (c_s = 0: no decay),
+//   G13: alpha^{n+1} = max((alpha^n + alpha_loc dt/tau) / (1 + dt/tau), alpha_loc).
+// Outputs: alpha_out; divv_out, curlv_out (|curl v|), aloc_out may be null.
+void orc_alpha_update(int64_t N, const double* pos, const double* vel, const double* acc, const double* m,
+                      const double* h, const double* rho, const double* omega, const double* u, const uint64_t* offs,
+                      const uint32_t* idx, const orc_box* box, const orc_params* p, double dt, const double* alpha_in,
+                      double* alpha_out, double* divv_out, double* curlv_out, double* aloc_out) {
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    for (int64_t a = 0; a < N; ++a) {
+        double gv[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // gv[i][j] = d_j v_i
+        double diva = 0.0;
+        for (uint64_t s = offs[a]; s < offs[a + 1]; ++s) {
+            uint32_t b = idx[s];
+            if ((int64_t)b == a) continue;
+            Sep sp = separation(x, y, z, a, b, *box);
+            double r = std::sqrt(sp.d2);
+            if (!(r > 0.0)) continue;
+            const double rh[3] = {sp.dx / r, sp.dy / r, sp.dz / r};
+            const double Fa = Fab(r, h[a]);
+            for (int i = 0; i < 3; ++i) {
+                const double dv = vel[i * N + a] - vel[i * N + b];
+                for (int j = 0; j < 3; ++j) gv[i][j] += m[b] * dv * rh[j] * Fa;
+                diva += m[b] * (acc[i * N + a] - acc[i * N + b]) * rh[i] * Fa;
+            }
+        }
+        const double norm = -1.0 / (omega[a] * rho[a]);
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) gv[i][j] *= norm;
+        diva *= norm;
+        const double divv = gv[0][0] + gv[1][1] + gv[2][2];
+        const double cx = gv[2][1] - gv[1][2], cy = gv[0][2] - gv[2][0], cz = gv[1][0] - gv[0][1];
+        const double curl2 = cx * cx + cy * cy + cz * cz;
+        double trs = 0.0;
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) trs += gv[i][j] * gv[j][i];
+        const double ddivdt = diva - trs;
+        const double den = divv * divv + curl2;
+        const double xi = den > 0.0 ? divv * divv / den : 1.0;
+        const double A = xi * std::max(-ddivdt, 0.0);
+        double P, cs;
+        eos(*p, rho[a], u[a], x[a], y[a], P, cs);
+        double aloc;
+        if (cs > 0.0) aloc = std::min(std::max(10.0 * h[a] * h[a] * A / (cs * cs), p->alpha_min), p->alpha_max);
+        else aloc = A > 0.0 ? p->alpha_max : p->alpha_min;
+        const double xdt = cs > 0.0 ? dt * p->sigma_decay * cs / h[a] : 0.0;                  // dt / tau
+        alpha_out[a] = std::max((alpha_in[a] + aloc * xdt) / (1.0 + xdt), aloc);                // G13
+        if (divv_out) divv_out[a] = divv;
+        if (curlv_out) curlv_out[a] = std::sqrt(curl2);
+        if (aloc_out) aloc_out[a] = aloc;
+    }
+}
+
+// per-particle alpha for the next orc_forces call (null = the constant p->alpha_av of reading A10); test infrastructure,
+// single-threaded: a file-level selector like the kernel choice
+const double* g_alpha = nullptr;
+void orc_set_alpha(const double* alpha) { g_alpha = alpha; }
+
 // ---- O8 + O9: forces (Eq. 3-6, 8-10; minus sign G1, q inside the sum G2), per-particle CFL
 // candidates (G8; v_sig^dt reading A12) and their global minimum.
 double orc_forces(int64_t N, const double* pos, const double* vel, const double* m, const double* h,
@@ -547,8 +617,8 @@ double orc_forces(int64_t N, const double* pos, const double* vel, const double*
             double rx = sp.dx / r, ry = sp.dy / r, rz = sp.dz / r;
             double dvx = vx[a] - vx[b], dvy = vy[a] - vy[b], dvz = vz[a] - vz[b];
             double w = dvx * rx + dvy * ry + dvz * rz;      // v_ab . r_hat_ab
-            double vsa = p->alpha_av * cs[a] + p->beta_av * std::fabs(w);   // Eq. 6
-            double vsb = p->alpha_av * cs[b] + p->beta_av * std::fabs(w);
+            double vsa = (g_alpha ? g_alpha[a] : p->alpha_av) * cs[a] + p->beta_av * std::fabs(w);   // Eq. 6
+            double vsb = (g_alpha ? g_alpha[b] : p->alpha_av) * cs[b] + p->beta_av * std::fabs(w);
             double qa = (w < 0.0) ? -0.5 * rho[a] * vsa * w : 0.0;          // Eq. 5
             double qb = (w < 0.0) ? -0.5 * rho[b] * vsb * w : 0.0;
             double Fa = Fab(r, h[a]), Fb = Fab(r, h[b]);                    // Eq. 10
@@ -585,10 +655,13 @@ double orc_forces(int64_t N, const double* pos, const double* vel, const double*
 // forces. h is in/out (h^n in, converged h out). mode 0 = brute-force neighbour search, 1 = cell grid.
 // Returns restarts >= 0, or -1 (h iteration cap), -2 (restart cap). If offs_out/idx_out are non-null and
 // cap suffices they receive the final cache.
+// alpha (may be null): per-particle shock-switch alpha, in/out; a_prev = a^n (null: zeros) and dt_alpha = the step's dt
+// enter G12-G13, evaluated between the smoothing-length update and the derivatives (Fig. G1).
 static int32_t evaluate_impl(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
                              double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
                              double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out,
-                             std::vector<uint64_t>& offs, std::vector<uint32_t>& idx) {
+                             std::vector<uint64_t>& offs, std::vector<uint32_t>& idx, double* alpha = nullptr,
+                             const double* a_prev = nullptr, double dt_alpha = 0.0) {
     offs.assign(N + 1, 0);
     idx.clear();
     std::vector<double> hn(h, h + N), hnew(N);
@@ -606,7 +679,16 @@ static int32_t evaluate_impl(int64_t N, const double* pos, const double* vel, co
         if (++restarts > p->max_restarts) return -2;
     }
     std::memcpy(h, hnew.data(), N * sizeof(double));
+    if (p->av_switch && alpha) {
+        std::vector<double> zeros, anew(N);
+        if (!a_prev) { zeros.assign(3 * N, 0.0); a_prev = zeros.data(); }
+        orc_alpha_update(N, pos, vel, a_prev, m, h, rho, omega, u, offs.data(), idx.data(), box, p, dt_alpha, alpha,
+                         anew.data(), nullptr, nullptr, nullptr);
+        std::memcpy(alpha, anew.data(), N * sizeof(double));
+        g_alpha = alpha;
+    }
     double dt = orc_forces(N, pos, vel, m, h, rho, omega, u, offs.data(), idx.data(), box, p, acc, dudt);
+    g_alpha = nullptr;
     if (dt_out) *dt_out = dt;
     if (n_neigh_out) *n_neigh_out = (int64_t)idx.size();
     return restarts;
@@ -618,6 +700,14 @@ int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const doub
     std::vector<uint64_t> offs;
     std::vector<uint32_t> idx;
     return evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, dt_out, n_neigh_out, offs, idx);
+}
+// the same with the shock switch: alpha in/out (white step: a^n = 0, dt = 0, so alpha rises to alpha_loc at once)
+int32_t orc_evaluate_alpha(int64_t N, const double* pos, const double* vel, const double* m, const double* u,
+                           double* h, const orc_box* box, const orc_params* p, int32_t mode, double* rho,
+                           double* omega, double* acc, double* dudt, double* dt_out, int64_t* n_neigh_out, double* alpha) {
+    std::vector<uint64_t> offs;
+    std::vector<uint32_t> idx;
+    return evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, dt_out, n_neigh_out, offs, idx, alpha);
 }
 
 // ---- O10: one leapfrog KDK step (G1-G5; order of Fig. G1; u integrated
@@ -632,9 +722,9 @@ int32_t orc_evaluate(int64_t N, const double* pos, const double* vel, const doub
 // dv = dt/2 (a_new - a_previous) is applied again. CFL multiplier (G9-G10): *cfl_mult is
 // halved after a step that re-cycled, else relaxed by (1 + stiff * mult) / (1 + stiff) (reading A16: lambda_stiff is
 // not given in the paper; it is a parameter); dt_next = mult * G8, as both terms of G8 are linear in the C's.
-int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
-                  double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
-                  double* omega, double* dt_next, double* cfl_mult, int32_t* n_recycle) {
+static int32_t step_impl(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                         double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                         double* omega, double* dt_next, double* cfl_mult, int32_t* n_recycle, double* alpha) {
     std::vector<double> a_old(acc, acc + 3 * N), du_old(dudt, dudt + N);
     for (int c = 0; c < 3; ++c) {
         double L = box->hi[c] - box->lo[c];
@@ -657,7 +747,8 @@ int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* 
     std::vector<uint64_t> offs;
     std::vector<uint32_t> idx;
     double dt_raw = 0.0;
-    int32_t rc = evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, &dt_raw, nullptr, offs, idx);   // G4
+    int32_t rc = evaluate_impl(N, pos, vel, m, u, h, box, p, mode, rho, omega, acc, dudt, &dt_raw, nullptr, offs, idx,
+                               alpha, a_old.data(), dt);   // G4 (with G12-G13 before it if the switch is on)
     if (rc < 0) return rc;
     int32_t recycles = 0;
     for (;;) {
@@ -681,7 +772,9 @@ int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* 
         ++recycles;
         a_old.assign(acc, acc + 3 * N);
         du_old.assign(dudt, dudt + N);
+        if (p->av_switch && alpha) g_alpha = alpha;      // alpha is not evolved again within a step
         dt_raw = orc_forces(N, pos, vel, m, h, rho, omega, u, offs.data(), idx.data(), box, p, acc, dudt);
+        g_alpha = nullptr;
     }
     double mult = cfl_mult ? *cfl_mult : 1.0;
     if (p->eps_v > 0.0) {
@@ -691,6 +784,17 @@ int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* 
     if (dt_next) *dt_next = mult * dt_raw;
     if (n_recycle) *n_recycle = recycles;
     return rc;
+}
+
+int32_t orc_step2(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                  double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                  double* omega, double* dt_next, double* cfl_mult, int32_t* n_recycle) {
+    return step_impl(N, pos, vel, m, u, h, acc, dudt, box, p, mode, dt, rho, omega, dt_next, cfl_mult, n_recycle, nullptr);
+}
+int32_t orc_step3(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
+                  double* dudt, const orc_box* box, const orc_params* p, int32_t mode, double dt, double* rho,
+                  double* omega, double* dt_next, double* cfl_mult, int32_t* n_recycle, double* alpha) {
+    return step_impl(N, pos, vel, m, u, h, acc, dudt, box, p, mode, dt, rho, omega, dt_next, cfl_mult, n_recycle, alpha);
 }
 
 int32_t orc_step(int64_t N, double* pos, double* vel, const double* m, double* u, double* h, double* acc,
