@@ -91,6 +91,15 @@ typedef struct {
                            sibling leaves; the leaf groups / traversal buckets are those reduced leaves (a leaf that
                            holds more than group_max particles is split by the group_max rule). The A/B variant of
                            SURVEY.md 8(f) item 1; results do not depend on it, the speed does (Fig. 16) */
+  /* Shock switch (G11-G13; runscript values PAPER.md:1412-1415; reading A18 for
+   * alpha_loc and tau, which the paper leaves to Price et al. 2018). */
+  int32_t av_switch;    /* 0  (constant alpha_av, reading A10); 1: per-particle alpha_a, starting at alpha_min, updated by
+                           the implicit step G13 between the smoothing-length update and the derivatives of every
+                           evaluation (a standalone sph_compute_forces uses dt = 0 and the stored a^n)               */
+  int32_t reserved4;
+  double alpha_min;     /* 0.0 */
+  double alpha_max;     /* 1.0 */
+  double sigma_decay;   /* 0.1  PAPER.md:1412: tau = h / (sigma_decay c_s) */
 } sph_params;
 
 /* Device-memory hooks so that the host framework (PyTorch's caching allocator) owns device memory.
@@ -208,6 +217,8 @@ int sph_get_neighbours_range(sph_ctx* ctx, sph_mem mem, int64_t first, int64_t c
  * N; leaf j holds the sorted slots [id_map[j], id_map[j+1]), Alg. 2). Buffers must hold N and N + 1
  * entries; either may be NULL. */
 int sph_get_leaves(sph_ctx* ctx, sph_mem mem, int64_t* n_leaves, uint64_t* leaf_codes, uint32_t* id_map);
+/* Shock-switch alpha_a in ORIGINAL particle order (sph_params.av_switch = 1; SPH_ERR_ORDER otherwise). */
+int sph_get_alpha(sph_ctx* ctx, sph_mem mem, double* alpha);
 int sph_get_stats(sph_ctx* ctx, sph_stats* out);
 int sph_reset_timers(sph_ctx* ctx);
 const char* sph_last_error(const sph_ctx* ctx);

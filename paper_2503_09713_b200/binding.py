@@ -22,7 +22,7 @@ STATUS = {0: "SPH_OK", -1: "SPH_ERR_ARG", -2: "SPH_ERR_DEVICE", -3: "SPH_ERR_OOM
 # every symbol include/sph_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["sph_default_params", "sph_init", "sph_init_ex", "sph_build_tree", "sph_compute_density",
            "sph_compute_forces", "sph_step_leapfrog", "sph_set_fields", "sph_get_fields", "sph_get_keys_perm",
-           "sph_get_tree", "sph_get_neighbours", "sph_get_neighbours_range", "sph_get_leaves", "sph_get_stats", "sph_reset_timers", "sph_last_error", "sph_free",
+           "sph_get_tree", "sph_get_neighbours", "sph_get_neighbours_range", "sph_get_leaves", "sph_get_alpha", "sph_get_stats", "sph_reset_timers", "sph_last_error", "sph_free",
            "sph_measure_fp64_peak"]
 
 
@@ -43,7 +43,8 @@ class Params(C.Structure):
                 ("max_restarts", C.c_int32), ("eos", C.c_int32), ("kernel", C.c_int32), ("cs0", C.c_double),
                 ("r0", C.c_double), ("q", C.c_double), ("GM", C.c_double), ("soft", C.c_double),
                 ("centre", C.c_double * 3), ("eps_v", C.c_double), ("lambda_stiff", C.c_double),
-                ("max_recycle", C.c_int32), ("group_max", C.c_int32), ("morton_bits", C.c_int32), ("leaf_reduction", C.c_int32)]
+                ("max_recycle", C.c_int32), ("group_max", C.c_int32), ("morton_bits", C.c_int32), ("leaf_reduction", C.c_int32), ("av_switch", C.c_int32),
+                ("reserved4", C.c_int32), ("alpha_min", C.c_double), ("alpha_max", C.c_double), ("sigma_decay", C.c_double)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -97,6 +98,7 @@ def load():
         lib.sph_get_neighbours.argtypes = [vp, C.c_int, vp, vp, C.c_uint64]
         lib.sph_get_neighbours_range.argtypes = [vp, C.c_int, i64, i64, vp, vp, C.c_uint64]
         lib.sph_get_leaves.argtypes = [vp, C.c_int, C.POINTER(C.c_int64), vp, vp]
+        lib.sph_get_alpha.argtypes = [vp, C.c_int, vp]
         lib.sph_get_stats.argtypes = [vp, C.POINTER(Stats)]
         lib.sph_measure_fp64_peak.argtypes = [C.POINTER(dbl), vp]
         _lib = lib
@@ -134,6 +136,8 @@ def params_for(w, **kw) -> Params:
         extra.update(morton_bits=w.morton_bits)
     if getattr(w, "leaf_reduction", 0):
         extra.update(leaf_reduction=w.leaf_reduction)
+    if getattr(w, "av_switch", 0):
+        extra.update(av_switch=1)
     extra.update(kw)
     return default_params(**extra)
 
@@ -327,6 +331,12 @@ class Sim:
         idx = np.empty(int(offs[-1] - offs[0]), dtype=np.uint32)
         self._check(self.lib.sph_get_neighbours_range(self.ctx, SPH_MEM_HOST, first, count, _ptr(offs), _ptr(idx), idx.size))
         return offs - offs[0], idx
+
+    def get_alpha(self):
+        """Shock-switch alpha_a in original order (av_switch = 1), as a numpy array."""
+        out = np.empty(self.n, dtype=np.float64)
+        self._check(self.lib.sph_get_alpha(self.ctx, SPH_MEM_HOST, _ptr(out)))
+        return out
 
     def get_leaves(self):
         """Reduced leaves of Alg. 1 (leaf_reduction >= 1): (leaf codes u64[n_leaf], id map u32[n_leaf + 1])."""

@@ -226,6 +226,7 @@ void sph_default_params(sph_params* p) {
     p->max_h_iter = 50; p->max_restarts = 50; p->eos = 0; p->kernel = 0;
     p->cs0 = 1.0; p->r0 = 1.0; p->q = 0.0; p->GM = 0.0; p->soft = 0.0;
     p->eps_v = 0.0; p->lambda_stiff = 2.0; p->max_recycle = 10; p->group_max = kGroup; p->morton_bits = 21;
+    p->av_switch = 0; p->alpha_min = 0.0; p->alpha_max = 1.0; p->sigma_decay = 0.1;
 }
 
 const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
@@ -294,6 +295,11 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     SPH_TRY(dalloc(c, &c->parent, 2 * n));
     SPH_TRY(dalloc(c, &c->visit, n));
     SPH_TRY(dalloc(c, &c->gflag, n)); SPH_TRY(dalloc(c, &c->gscan, n + 1)); SPH_TRY(dalloc(c, &c->grp_lo, n + 1));
+    if (c->p.av_switch) {
+        if (!(c->p.alpha_max >= c->p.alpha_min) || !(c->p.alpha_min >= 0.0) || !(c->p.sigma_decay >= 0.0))
+            return fail(c, SPH_ERR_ARG, "shock switch needs 0 <= alpha_min <= alpha_max and sigma_decay >= 0");
+        SPH_TRY(dalloc(c, &c->alpha, n)); SPH_TRY(dalloc(c, &c->alpha_alt, n)); SPH_TRY(dalloc(c, &c->acs, n));
+    }
     if (c->p.leaf_reduction >= 1) { SPH_TRY(dalloc(c, &c->xi_a, n)); SPH_TRY(dalloc(c, &c->xi_b, n)); SPH_TRY(dalloc(c, &c->lscan, n + 1)); }
     SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
     SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
@@ -333,6 +339,10 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
     }
     k_mass_uniform<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->cur.m, c->d_sc);
     c->launches++;
+    if (c->p.av_switch) {     // alpha starts at alpha_min; the white step's G13 (dt = 0) raises it to alpha_loc
+        k_fill<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->alpha, c->p.alpha_min);
+        c->launches++;
+    }
     SPH_CUDA(c, cudaGetLastError());
     SPH_TRY(read_scalars(c));
     c->uniform_mass = (c->h_sc->mass_nonuniform == 0u);
@@ -406,6 +416,8 @@ static int forces_eval(sph_ctx* c) {
 int sph_compute_forces(sph_ctx* c) {
     SPH_TRY(check_ctx(c));
     DeviceGuard dg(c);
+    c->alpha_pending = true;      // standalone evaluation: G13 with dt = 0 and the stored a^n
+    c->in_step = false;
     SPH_TRY(forces_eval(c));
     // standalone evaluation (and the white step): the result becomes a^n, du/dt^n of the next predictor
     StageTimer t(c, ST_LEAPFROG);
@@ -424,7 +436,11 @@ int sph_step_leapfrog(sph_ctx* c, double dt, double* dt_used) {
     c->state = S_FIELDS;
     SPH_TRY(sph_build_tree(c));
     SPH_TRY(sph_compute_density(c));
-    SPH_TRY(forces_eval(c));
+    c->alpha_pending = true;      // G12-G13 once per step, before the derivatives; re-cycles keep alpha
+    c->in_step = true;
+    const int rc_f = forces_eval(c);
+    c->in_step = false;
+    SPH_TRY(rc_f);
     const bool check = c->p.eps_v > 0.0;
     { StageTimer t(c, ST_LEAPFROG); SPH_TRY(launch_correct(c, check)); }
     c->recycles_last = 0;
@@ -608,6 +624,20 @@ int sph_get_neighbours_range(sph_ctx* c, sph_mem mem, int64_t first, int64_t cou
 int sph_get_neighbours(sph_ctx* c, sph_mem mem, uint64_t* offs, uint32_t* idx, uint64_t cap) {
     SPH_TRY(check_ctx(c));
     return sph_get_neighbours_range(c, mem, 0, c->N, offs, idx, cap);
+}
+
+int sph_get_alpha(sph_ctx* c, sph_mem mem, double* alpha) {
+    SPH_TRY(check_ctx(c));
+    DeviceGuard dg(c);
+    if (!c->p.av_switch) return fail(c, SPH_ERR_ORDER, "sph_get_alpha needs sph_params.av_switch = 1");
+    if (!alpha) return SPH_ERR_ARG;
+    double* stage = nullptr;
+    int rc = copy_out(c, mem, c->alpha, alpha, 1, &stage);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (stage) dfree(c, stage);
+    if (rc != SPH_OK) return rc;
+    if (e != cudaSuccess) return fail(c, SPH_ERR_DEVICE, "stream sync failed: %s", cudaGetErrorString(e));
+    return SPH_OK;
 }
 
 int sph_get_leaves(sph_ctx* c, sph_mem mem, int64_t* n_leaves, uint64_t* leaf_codes, uint32_t* id_map) {

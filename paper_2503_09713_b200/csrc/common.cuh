@@ -103,6 +103,10 @@ struct sph_ctx {
     double *rho = nullptr, *omega = nullptr, *P = nullptr, *cs = nullptr, *A = nullptr;   // A = 1/(rho^2 Omega)
     double *nax = nullptr, *nay = nullptr, *naz = nullptr, *ndu = nullptr;                // a^{n+1}, du/dt^{n+1}
     double* hnew = nullptr;                                                               // Newton output
+    // shock switch (sph_params.av_switch): alpha_a in sorted order (two sets: the permute writes the other), alpha c_s
+    double *alpha = nullptr, *alpha_alt = nullptr, *acs = nullptr;
+    bool alpha_pending = false;         // the next force evaluation starts with the G13 update
+    bool in_step = false;               // inside sph_step_leapfrog (the G13 update takes the step's dt, else 0)
     uint64_t *key = nullptr, *key_alt = nullptr;
     uint32_t *val = nullptr, *val_alt = nullptr;
     // radix sort scratch
@@ -202,6 +206,7 @@ int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
 int launch_density(sph_ctx* c);                                // density.cu
 int launch_forces(sph_ctx* c);                                 // forces.cu
+int launch_alpha(sph_ctx* c, const double* dtp);               // alpha.cu  G12-G13 update of alpha_a, alpha c_s
 int launch_predict(sph_ctx* c);                                // leapfrog.cu
 int launch_correct(sph_ctx* c, bool with_check);                           // leapfrog.cu
 int launch_hmax(sph_ctx* c);                                   // leapfrog.cu  max h^n -> d_sc->h_max

@@ -11,6 +11,8 @@ struct PermArgs {
     double* dst[kNumF64Fields];
     const uint32_t* src_id;
     uint32_t* dst_id;
+    const double* src_alpha;   // shock-switch alpha_a (null unless sph_params.av_switch)
+    double* dst_alpha;
 };
 
 // Each thread moves one particle: 14 independent gathers in flight, 14 coalesced stores.
@@ -25,6 +27,7 @@ __global__ void __launch_bounds__(256) k_permute(int64_t N, const uint32_t* __re
 #pragma unroll
     for (int f = 0; f < kNumF64Fields; ++f) a.dst[f][i] = v[f];
     a.dst_id[i] = id;
+    if (a.src_alpha) a.dst_alpha[i] = __ldg(a.src_alpha + s);
 }
 
 int launch_permute(sph_ctx* c) {
@@ -35,10 +38,13 @@ int launch_permute(sph_ctx* c) {
     for (int f = 0; f < kNumF64Fields; ++f) { a.src[f] = sp[f]; a.dst[f] = dp[f]; }
     a.src_id = s.id;
     a.dst_id = d.id;
+    a.src_alpha = c->alpha;
+    a.dst_alpha = c->alpha_alt;
     k_permute<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->val, a);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     Fields t = c->cur; c->cur = c->alt; c->alt = t;
+    double* ta = c->alpha; c->alpha = c->alpha_alt; c->alpha_alt = ta;
     return SPH_OK;
 }
 

@@ -57,6 +57,7 @@ class Workload:
     eps_v: float | None = None  # leapfrog corrector check G7; None / 0 = off
     kernel: int = 0  # SPH kernel: 0 = M4 (all BASELINE configs), 1 = M5, 2 = M6, 3/4/5 = Wendland C2/C4/C6
     morton_bits: int = 21  # grid bits per axis of the Morton code: 21, or 10 = the paper's 30-bit variant
+    av_switch: int = 0  # 1 = shock-switch alpha evolution (G11-G13) instead of the constant alpha
     leaf_reduction: int = 0  # 0 = off; k >= 1: leaf groups from the paper's Alg. 1 with n_red = k - 1 passes
 
     @property

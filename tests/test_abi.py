@@ -27,7 +27,7 @@ def _declared_functions():
 def test_library_exports_every_declared_symbol(lib):
     from paper_2503_09713_b200 import binding
     names = _declared_functions()
-    assert len(names) >= 19
+    assert len(names) >= 20
     for n in names:
         assert hasattr(lib, n), f"{n} declared in sph_b200.h but not exported"
     assert sorted(binding.SYMBOLS) == names
@@ -40,7 +40,8 @@ def test_default_params_match_header_citations(lib):
     assert (p.alpha_av, p.beta_av, p.beta_u, p.c_cour, p.c_force) == (1.0, 2.0, 1.0, 0.3, 0.25)
     assert p.gamma == pytest.approx(5.0 / 3.0) and p.max_h_iter == 50 and p.max_restarts == 50 and p.eos == 0
     assert (p.eps_v, p.lambda_stiff, p.max_recycle) == (0.0, 2.0, 10)      # corrector re-cycle off by default
-    assert C.sizeof(binding.Params) == 10 * 8 + 4 * 4 + 5 * 8 + 3 * 8 + 2 * 8 + 4 * 4
+    assert C.sizeof(binding.Params) == 10 * 8 + 4 * 4 + 5 * 8 + 3 * 8 + 2 * 8 + 4 * 4 + 2 * 4 + 3 * 8
+    assert (p.av_switch, p.alpha_min, p.alpha_max, p.sigma_decay) == (0, 0.0, 1.0, 0.1)
     assert (p.group_max, p.morton_bits) == (32, 21)
     assert C.sizeof(binding.Box) == 6 * 8 + 3 * 4 + 4   # padded to 8
 

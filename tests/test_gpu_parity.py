@@ -1009,3 +1009,48 @@ def test_leaf_reduction_variant_sampled_parity_128():
         _slot_sample_parity(sim, gperm, s0, 1024, w.pos, w.vel, w.u, w.h0, w.mass, box, p, f)
     _stepped_parity(w, sim, 2, (2,), (0.0, 0.5))
     sim.close()
+
+
+@pytest.mark.parametrize("make", [
+    lambda: W.sod(16, 12),
+    lambda: W.cube(14, jitter=0.08, vel_amp=0.3, seed=9),
+], ids=["sod_small", "cube_compressive"])
+def test_shock_switch_parity(make):
+    """sph_params.av_switch = 1 (G11-G13; reading A18): per-particle alpha_a from the implicit step
+    G13, used in Eq. 6 for both particles of a pair. White step (dt = 0: alpha rises to alpha_loc) and a five-step
+    trajectory follow the oracle: alpha, fields and dt."""
+    w = make()
+    w.av_switch = 1
+    sim = _sim(w)
+    s = O.State(w, "grid")
+    f = _np(sim.get_fields())
+    assert np.max(np.abs(sim.get_alpha() - s.alpha)) < 1e-9            # (zero where the initial velocity vanishes)
+    assert np.max(np.abs(f["acc"] - s.acc)) <= TOL_ACC * np.abs(s.acc).max()
+    assert np.max(np.abs(f["dudt"] - s.dudt)) <= TOL_ACC * max(np.abs(s.dudt).max(), 1e-12)
+    assert sim.stats()["dt"] == pytest.approx(s.dt, rel=1e-12)
+    for _ in range(5):
+        assert sim.step_leapfrog(want_dt=True) == pytest.approx(s.step(), rel=1e-9)
+        assert np.max(np.abs(sim.get_alpha() - s.alpha)) < 1e-7
+    g = _np(sim.get_fields())
+    assert np.max(np.abs(g["pos"] - s.pos)) < 1e-11 and np.max(np.abs(g["vel"] - s.vel)) < 1e-9
+    assert np.max(np.abs(g["u"] - s.u)) < 1e-9 * np.abs(s.u).max()
+    assert np.max(np.abs(g["acc"] - s.acc)) < 1e-7 * np.abs(s.acc).max()
+    a = sim.get_alpha()
+    assert np.all((a >= 0.0) & (a <= 1.0)) and a.max() > 0.05
+    sim.close()
+
+
+def test_shock_switch_constant_alpha_limit():
+    """alpha_min = alpha_max = 1 pins alpha_a = 1 for every particle: the switch variant of the force kernel (staged
+    alpha c_s row) then reproduces the constant-alpha kernel to rounding."""
+    from paper_2503_09713_b200 import binding as B
+    w = W.random_cloud(3000, seed=5, periodic=True, clustered=False)
+    a = _sim(w)
+    b = _sim(w, params=B.params_for(w, av_switch=1, alpha_min=1.0, alpha_max=1.0))
+    for _ in range(2):
+        a.step_leapfrog(); b.step_leapfrog()
+    fa, fb = _np(a.get_fields()), _np(b.get_fields())
+    assert np.all(b.get_alpha() == 1.0)
+    for k in ("pos", "vel", "u", "acc", "dudt"):
+        assert np.allclose(fa[k], fb[k], rtol=1e-12, atol=1e-14 * np.abs(fa[k]).max()), k
+    a.close(); b.close()
