@@ -139,6 +139,10 @@ typedef struct {
   double cfl_mult;         /* CFL multiplier lambda_CFL applied to the next internal dt                     */
   int64_t density_sweeps;  /* sweeps over the neighbour lists executed by the last density pass, summed over
                               particles: Newton sweeps + the closing pass at the converged h (Omega)         */
+  int64_t n_inner;         /* entries of the cache's inner list segments (within R_kern 1.02 max(h_a, h_b) at build
+                              time); the other n_neighbours - n_inner shell entries are skipped by density and forces
+                              until some smoothing length has grown by 2 %                              */
+  int64_t n_grew;          /* particles whose h grew past that bound in the last density pass                        */
 } sph_stats;
 
 void sph_default_params(sph_params* p);

@@ -64,7 +64,7 @@ class Stats(C.Structure):
                 ("t", C.c_double), ("bytes_allocated", C.c_int64), ("cand_max", C.c_int32), ("groups_fallback", C.c_int32),
                 ("chunks_shared", C.c_int32), ("share_chunk", C.c_int32), ("sort_passes", C.c_int32),
                 ("sort_tie_max", C.c_int32), ("recycles", C.c_int32), ("reserved", C.c_int32), ("cfl_mult", C.c_double),
-                ("density_sweeps", C.c_int64)]
+                ("density_sweeps", C.c_int64), ("n_inner", C.c_int64), ("n_grew", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -29,6 +29,7 @@ struct AlphaIn {
     const GroupRec* ginfo;
     const uint32_t* cslot;
     const uint32_t* cnt;
+    const uint32_t* cnt_in;
     const uint64_t* lstart;
     const uint16_t* lists;
 };
@@ -58,9 +59,8 @@ __global__ void __launch_bounds__(kAlphaWarps * 32, 2) k_alpha(AlphaIn in, Alpha
     const double ha = in.h[a], hinv = 1.0 / ha;
     const double ca4 = kern_cnorm(K) * (hinv * hinv) * (hinv * hinv);
     const uint16_t* li = in.lists + in.lstart[a];
-    const uint32_t n = pv ? in.cnt[a] : 0u;
+    const uint32_t n = pv ? in.cnt[a] : 0u;      // all entries are read: inner, then shell
     double gv[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, diva = 0.0;
-    uint32_t kcur = 0;
     for (uint32_t c0 = 0; c0 < nc; c0 += kAChunk) {
         const uint32_t c1 = min(nc, c0 + (uint32_t)kAChunk);
         if (c0 > 0) __syncthreads();
@@ -74,11 +74,10 @@ __global__ void __launch_bounds__(kAlphaWarps * 32, 2) k_alpha(AlphaIn in, Alpha
         }
         asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
         __syncthreads();
-        // lists ascend: the entries of this chunk are a contiguous run of the particle's list, split over the octet
-        for (;;) {
-            const uint32_t k = kcur + sl;
+        // the octet's lanes split the list; entries outside the staged chunk are skipped (one chunk in the usual case)
+        for (uint32_t k = sl;; k += 8u) {
             const uint32_t cl = (k < n) ? (uint32_t)li[k] : 0xffffffffu;
-            const bool act = cl < c1;
+            const bool act = cl - c0 < c1 - c0;
             if (act) {
                 const uint32_t b = cl - c0;
                 double dx = xa - asm_[b], dy = ya - asm_[kAChunk + b], dz = za - asm_[2 * kAChunk + b];
@@ -103,11 +102,7 @@ __global__ void __launch_bounds__(kAlphaWarps * 32, 2) k_alpha(AlphaIn in, Alpha
                     }
                 }
             }
-            const unsigned om = __ballot_sync(0xffffffffu, act) & (0xffu << (8u * sub));
-            kcur += (uint32_t)__popc(om);
-            const uint32_t kn = kcur + sl;
-            const bool more = kn < n && (uint32_t)li[kn] < c1;
-            if (__ballot_sync(0xffffffffu, more) == 0u) break;
+            if (__ballot_sync(0xffffffffu, k + 8u < n) == 0u) break;
         }
     }
 #pragma unroll
@@ -172,7 +167,7 @@ int launch_alpha(sph_ctx* c, const double* dtp) {
     in.x = c->cur.x; in.y = c->cur.y; in.z = c->cur.z; in.vx = c->cur.vx; in.vy = c->cur.vy; in.vz = c->cur.vz;
     in.ax = c->cur.ax; in.ay = c->cur.ay; in.az = c->cur.az; in.m = c->cur.m; in.h = c->cur.h; in.rho = c->rho;
     in.omega = c->omega; in.cs = c->cs;
-    in.grp_lo = c->grp_lo; in.ginfo = c->ginfo; in.cslot = c->cslot; in.cnt = c->cnt; in.lstart = c->lstart; in.lists = c->lists;
+    in.grp_lo = c->grp_lo; in.ginfo = c->ginfo; in.cslot = c->cslot; in.cnt = c->cnt; in.cnt_in = c->cnt_in; in.lstart = c->lstart; in.lists = c->lists;
     switch (c->p.kernel) {
         case 0: return alpha_launch_k<0>(c, in, aa, dtp);
         case 1: return alpha_launch_k<1>(c, in, aa, dtp);

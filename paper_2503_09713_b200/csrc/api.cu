@@ -301,7 +301,7 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
         SPH_TRY(dalloc(c, &c->alpha, n)); SPH_TRY(dalloc(c, &c->alpha_alt, n)); SPH_TRY(dalloc(c, &c->acs, n));
     }
     if (c->p.leaf_reduction >= 1) { SPH_TRY(dalloc(c, &c->xi_a, n)); SPH_TRY(dalloc(c, &c->xi_b, n)); SPH_TRY(dalloc(c, &c->lscan, n + 1)); }
-    SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
+    SPH_TRY(dalloc(c, &c->cnt, n + 1)); SPH_TRY(dalloc(c, &c->cnt_in, n + 1)); SPH_TRY(dalloc(c, &c->grow, n + 1)); SPH_TRY(dalloc(c, &c->lstart, n)); SPH_TRY(dalloc(c, &c->offs, n + 1));
     SPH_TRY(dalloc(c, &c->trav_scratch, trav_scratch_entries()));
     SPH_TRY(dalloc(c, &c->trav_hit_scratch, trav_hit_scratch_entries()));
     SPH_TRY(dalloc(c, &c->corr_part, 2 * (size_t)div_up(N, 256) + 2));
@@ -697,7 +697,7 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
     out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
     out->sort_passes = c->last_sort_passes; out->sort_tie_max = (int32_t)s.tie_max;
-    out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult; out->density_sweeps = (int64_t)s.sweeps;
+    out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult; out->density_sweeps = (int64_t)s.sweeps; out->n_inner = (int64_t)s.n_inner; out->n_grew = (int64_t)s.n_grew;
     return SPH_OK;
 }
 

@@ -17,6 +17,12 @@
 namespace sph {
 
 constexpr int kGroup = 32;          // leaf-group size bound: one warp lane per particle of a group
+// Neighbour lists are split at R_kern (1 + kShellEps) max(h_a, h_b) (h at cache-build time): the entries beyond it
+// (the shell kept for the chi tolerance) can only contribute once some smoothing length has grown by
+// more than kShellEps since the build; density and forces skip them until then
+constexpr double kShellEps = 0.02;
+// growth beyond which the shell entries are read: (1 + kShellEps) less the margins of the traversal's classification
+constexpr double kShellGrow = (1.0 + kShellEps) * (1.0 - 1e-5);
 // B-spline kernels (reading O6): 0 = M4 (cubic), 1 = M5 (quartic), 2 = M6 (quintic);
 // support radius in units of h and 3-D normalisation 1/pi, 1/(20 pi), 1/(120 pi)
 // 3, 4, 5 = Wendland C2, C4, C6 on the support radius 2h: f = t^4 (1 + 2q), t^6 (1 + 3q + 35/12 q^2),
@@ -81,6 +87,8 @@ struct DevScalars {
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
     unsigned int sort_redo;          // prefix-mode sort met a run of equal prefixes too long to repair: the tree kernels
                                      // of this build do nothing and the host sorts again with all eight passes
+    unsigned long long n_inner;      // inner entries of all lists (the rest are shell entries, neigh.cu)
+    unsigned long long n_grew;       // particles flagged by the last density pass (h' > kShellGrow h^n)
     unsigned long long sweeps;       // Newton sweeps + closing passes executed by the last density launch, summed over
                                      // particles (bench.py: measured flop count of k_density)
 };
@@ -130,6 +138,8 @@ struct sph_ctx {
     // neighbour cache, group-local (a4): per group a candidate array (sorted slots of the particles
     // that passed the traversal's prefilter) and per particle an ascending list of 16-bit indices into it
     uint32_t* cnt = nullptr;            // N+1  list length of each sorted slot
+    uint32_t* cnt_in = nullptr;         // N    of which inner entries (first segment of the list)
+    uint8_t* grow = nullptr;            // N    1 if the last density solve left h' > kShellGrow h^n for this slot
     uint64_t* lstart = nullptr;         // N    first entry of each slot's list in `lists`
     uint16_t* lists = nullptr;
     uint64_t list_cap = 0;
@@ -204,6 +214,7 @@ size_t trav_hit_scratch_entries();                              // neigh.cu  u16
 size_t trav_scratch_entries();                                  // neigh.cu  u32 entries of the traversal's scratch rows
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out);  // scan.cu
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out);        // scan.cu
+int launch_scan_groups(sph_ctx* c, const uint32_t* gflag, uint32_t* gscan, uint32_t* grp_lo, int64_t n);               // scan.cu
 int launch_density(sph_ctx* c);                                // density.cu
 int launch_forces(sph_ctx* c);                                 // forces.cu
 int launch_alpha(sph_ctx* c, const double* dtp);               // alpha.cu  G12-G13 update of alpha_a, alpha c_s

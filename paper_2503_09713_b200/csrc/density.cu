@@ -15,7 +15,7 @@
 namespace sph {
 
 constexpr int kDensWarps = 8;
-constexpr int kRegChunks = 12;    // 12 x 8 = 96 neighbours held in registers per octet (kernels of radius 2)
+constexpr int kRegChunks = 10;    // 10 x 8 = 80 inner neighbours held in registers per octet (kernels of radius 2)
 // M5 / M6 (radii 2.5 and 3: ~157 neighbours at h_fact 1.2 / 1.0) keep 20 x 8 = 160; their launches run 2 CTAs per SM
 template <int K> constexpr int kRegChunksK = (K == 1 || K == 2) ? 20 : kRegChunks;
 
@@ -80,7 +80,7 @@ __device__ __forceinline__ void kern_f_g(double q, double& f, double& g) {
         g = fma(q, df, 3.0 * f);
     }
 }
-struct DensOut { double h, rho, om; bool exceeded, noconv; int it; };
+struct DensOut { double h, rho, om; bool exceeded, noconv, grew; int it; };
 
 // UNIM: every candidate of the group has the same mass (checked while staging): the mass factors out of the sums
 // and the per-neighbour mass registers disappear.
@@ -90,7 +90,7 @@ template <bool WRAP, bool UNIM, bool GLOB, int K>
 __device__ __forceinline__ void octet_solve(double xa, double ya, double za, double ma, double h0, bool pv,
                                             const uint32_t* __restrict__ cs,
                                             const uint16_t* __restrict__ li, const uint32_t (&idx)[(kRegChunksK<K> + 1) / 2],
-                                            int n, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
+                                            int n, int ntot, unsigned sl, const double* __restrict__ sx, const double* __restrict__ sy,
                                             const double* __restrict__ sz, const double* __restrict__ sm,
                                             const DensBox& db, const DensPar& dp, DensOut& out) {
     double r[kRegChunksK<K>], mb[UNIM ? 1 : kRegChunksK<K>];
@@ -108,7 +108,10 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
         }
     }
     // sums over the list at smoothing length h: rs = sum m f(q), ss = sum m (3 f + q f')
-    auto sums = [&](double hinv, double& rho_sum, double& S) {
+    // `n` inner entries (registers, then re-gathered beyond them); the ntot - n shell entries lie beyond
+    // R_kern (1 + kShellEps) h0 and are only read while h exceeds kShellGrow h0 (exact: they contribute nothing below)
+    const double hlim = kShellGrow * h0;
+    auto sums = [&](double hcur, double hinv, double& rho_sum, double& S) {
         double rs = 0.0, ss = 0.0;
 #pragma unroll
         for (int c = 0; c < kRegChunksK<K>; ++c) {
@@ -131,6 +134,17 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
             rs = fma(mm, f, rs);
             ss = fma(mm, g, ss);
         }
+        if (hcur > hlim) {
+            for (int k = n + (int)sl; k < ntot; k += 8) {
+                uint32_t b = li[k];
+                if (GLOB) b = cs[b];
+                double f, g;
+                const double mm = UNIM ? 1.0 : sm[b];
+                kern_f_g<K>(sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, g);
+                rs = fma(mm, f, rs);
+                ss = fma(mm, g, ss);
+            }
+        }
         rs = octet_sum(rs);
         ss = octet_sum(ss);
         const double c3 = (UNIM ? m0 : 1.0) * kern_cnorm(K) * hinv * hinv * hinv;
@@ -145,7 +159,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     while (__any_sync(0xffffffffu, active)) {      // the four octets of a warp iterate together
         double rho_sum, S;
         const double hinv = 1.0 / h;                                // the one reciprocal of a sweep besides f / f'
-        sums(hinv, rho_sum, S);
+        sums(h, hinv, rho_sum, S);
         if (active) {
             ++it;
             const double hf = dp.hfact * hinv;
@@ -166,13 +180,14 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     }
     double rho_sum, S;
     const double hinv = 1.0 / h;
-    sums(hinv, rho_sum, S);
+    sums(h, hinv, rho_sum, S);
     const double hf = dp.hfact * hinv;
     const double rho_a = ma * hf * hf * hf;
     out.h = h;
     out.rho = rho_a;
     out.om = 1.0 + h / (3.0 * rho_a) * S;                           // Eq. 7 with dh/drho = -h/(3 rho)
     out.exceeded = exceeded;
+    out.grew = h > hlim;
     out.noconv = pv && !exceeded && !converged;
     out.it = it;
 }
@@ -182,7 +197,7 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) 
     const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ m, const double* __restrict__ hn, const uint32_t* __restrict__ grp_lo,
     const GroupRec* __restrict__ ginfo, const uint32_t* __restrict__ cslot, const uint32_t* __restrict__ cnt,
-    const uint64_t* __restrict__ lstart, const uint16_t* __restrict__ lists, DensBox db, DensPar dp, uint32_t ncap,
+    const uint32_t* __restrict__ cnt_in, uint8_t* __restrict__ grow, const uint64_t* __restrict__ lstart, const uint16_t* __restrict__ lists, DensBox db, DensPar dp, uint32_t ncap,
     uint32_t nc_lo, uint32_t nc_hi,
     double* __restrict__ hout, double* __restrict__ rho, double* __restrict__ omega, DevScalars* sc) {
     extern __shared__ __align__(16) double dsm[];
@@ -206,7 +221,7 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) 
     const uint32_t a = glo + (pv ? q : 0u);
     const double xa = x[a], ya = y[a], za = z[a], ma = m[a], h0 = hn[a];
     const uint16_t* li = lists + lstart[a];
-    const int n = pv ? (int)cnt[a] : 0;
+    const int ntot = pv ? (int)cnt[a] : 0, n = pv ? (int)cnt_in[a] : 0;
 
     // ---- stage the candidate array (slots are mostly runs of consecutive indices: coalesced sectors) ----
     if (!GLOB) {
@@ -230,13 +245,14 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) 
     __syncthreads();
 
     DensOut o;
-    if (gwrap) octet_solve<true, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
-    else octet_solve<false, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, sl, sx, sy, sz, sm, db, dp, o);
+    if (gwrap) octet_solve<true, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, ntot, sl, sx, sy, sz, sm, db, dp, o);
+    else octet_solve<false, UNIM, GLOB, K>(xa, ya, za, ma, h0, pv, cs, li, idx, n, ntot, sl, sx, sy, sz, sm, db, dp, o);
 
     if (pv && sl == 0u) {
         hout[a] = o.h;
         rho[a] = o.rho;
         omega[a] = o.om;
+        grow[a] = o.grew ? 1 : 0;
     }
     const unsigned exc = __ballot_sync(0xffffffffu, pv && sl == 0u && o.exceeded);
     const unsigned ncv = __ballot_sync(0xffffffffu, sl == 0u && o.noconv);
@@ -247,15 +263,17 @@ __global__ void __launch_bounds__(kDensWarps * 32, (UNIM && (K == 0 || K >= 3)) 
     unsigned swp = (pv && sl == 0u) ? (unsigned)o.it + 1u : 0u;
 #pragma unroll
     for (int ofs = 16; ofs > 0; ofs >>= 1) swp += __shfl_xor_sync(0xffffffffu, swp, ofs);
+    const unsigned gm = __ballot_sync(0xffffffffu, pv && sl == 0u && o.grew);
     if (lane == 0) {
         if (exc) atomicAdd(&sc->n_exceeded, (unsigned)__popc(exc));
         if (ncv) atomicAdd(&sc->n_noconv, (unsigned)__popc(ncv));
         atomicMax(&sc->h_iter_max, itm);
         atomicAdd(&sc->sweeps, (unsigned long long)swp);
+        if (gm) atomicAdd(&sc->n_grew, (unsigned long long)__popc(gm));
     }
 }
 
-__global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; sc->sweeps = 0ull; }
+__global__ void k_density_reset(DevScalars* sc) { sc->n_exceeded = 0; sc->n_noconv = 0; sc->h_iter_max = 0; sc->sweeps = 0ull; sc->n_grew = 0ull; }
 
 template <bool UNIM, bool GLOB, int K>
 static int density_launch_k(sph_ctx* c, size_t smem, const DensBox& db, const DensPar& dp, uint32_t ncap, uint32_t lo,
@@ -263,7 +281,7 @@ static int density_launch_k(sph_ctx* c, size_t smem, const DensBox& db, const De
     if (!GLOB)   // per device: set on every launch
         SPH_CUDA(c, cudaFuncSetAttribute(k_density<UNIM, GLOB, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     k_density<UNIM, GLOB, K><<<(unsigned)c->n_groups, kDensWarps * 32, smem, c->stream>>>(
-        c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->lstart, c->lists, db, dp,
+        c->cur.x, c->cur.y, c->cur.z, c->cur.m, c->cur.h, c->grp_lo, c->ginfo, c->cslot, c->cnt, c->cnt_in, c->grow, c->lstart, c->lists, db, dp,
         ncap, lo, hi, c->hnew, c->rho, c->omega, c->d_sc);
     c->launches++;
     return SPH_OK;

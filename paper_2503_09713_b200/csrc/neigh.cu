@@ -58,6 +58,8 @@ struct TravBox {
     int periodic[3];
     double gg_pad;                       // absolute slack added to the conservative box test
     uint32_t gmax;                       // nodes with <= gmax particles are buckets (sph_params.group_max)
+    double kappa;                        // ((1 + kShellEps) / chi)^2 (at most 1): inner threshold / cache threshold
+    float kappa_f;
     const uint32_t* lscan;               // Alg. 1 variant (else null): scan of the removal mask; a bucket must also lie
                                          // inside one reduced leaf: lscan[hi + 1] == lscan[lo + 1]
 };
@@ -75,6 +77,7 @@ struct TravWarpSmem {
 
 struct TravOut {
     uint32_t* cnt;
+    uint32_t* cnt_in;
     uint64_t* lstart;
     uint16_t* lists;
     uint64_t list_cap;
@@ -117,8 +120,13 @@ struct GroupCtx {
     double gxl, gxh, gyl, gyh, gzl, gzh, ghm;
     double rc2g;          // (R_kern chi hmax_group)^2, for the per-candidate prefilter
     uint32_t nhit;        // per lane: hits so far (exact)
-    uint32_t wpos;        // per lane, buffered mode: store position in the lane's row
-    uint32_t nspill;      // per lane, buffered mode: hits of this group already spilled to the warp's global scratch
+    uint32_t nin;         // per lane: inner hits so far (exact)
+    uint32_t wpos;        // per lane: inner entries in the lane's row (DIRECT: inner entries written)
+    uint32_t cpos;        // per lane: shell entries in the lane's row, from the top (DIRECT: shell entries written)
+    uint32_t nspill;      // per lane, buffered mode: inner hits of this group already spilled to the warp's global scratch
+    uint32_t cspill;      // per lane, buffered mode: shell hits already spilled (they fill the scratch row from its top)
+    uint16_t* lcend;      // DIRECT: this lane's first shell entry in global memory (right after its inner entries)
+    float kin_a;          // per lane: kappa * ra2, the inner threshold of the query in scaled fp32
     bool hard_overflow;   // warp-uniform: a row could not spill any more (the group is walked a second time)
     uint16_t* hspill;     // warp-uniform: the warp's hit scratch (row p = hspill + p * kSpillCap belongs to lane p)
     uint32_t ncs;         // warp-uniform: candidates (prefilter survivors) so far
@@ -167,18 +175,52 @@ __device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigne
     return r;
 }
 
+// A particle's list has two segments: the INNER entries, d < R_kern (1 + kShellEps) max(h_a, h_b) at
+// build time, and the SHELL entries beyond (cached for the chi tolerance; they can only matter to a later kernel if some
+// h grew by more than kShellEps). The lane's row in shared memory fills from both ends: inner entries upwards from the
+// row start (ascending candidate index), shell entries downwards from the row top.
 template <bool DIRECT>
-__device__ __forceinline__ void record_hit(GroupCtx& G, uint32_t& wp, uint32_t local) {
+__device__ __forceinline__ void record_inner(GroupCtx& G, uint32_t& wp, uint32_t local) {
     if (DIRECT) {
-        if (G.can_write) G.lptr[G.nhit] = (uint16_t)local;
-        ++G.nhit;
+        if (G.can_write) G.lptr[G.wpos] = (uint16_t)local;
+        ++G.wpos;
     } else {
-        // wp = 32-bit shared-memory address of the lane's next free entry; the row has kHitSlack entries
-        // beyond kHitCap, so no capacity check is needed inside a bucket
+        // wp = 32-bit shared-memory address of the lane's next free entry; the row keeps kHitSlack entries free at the
+        // start of a bucket, so no capacity check is needed inside it
         // no "memory" clobber: the hit rows alias nothing that is read inside a bucket's test loop, and the loads of
         // the next candidates must be free to move above this store (stage2 closes the loop with a compiler barrier)
         asm volatile("st.shared.u16 [%0], %1;" :: "r"(wp), "h"((unsigned short)local));
         wp += 2u;
+    }
+}
+template <bool DIRECT>
+__device__ __forceinline__ void record_shell(GroupCtx& G, uint32_t& wq, uint32_t local) {
+    if (DIRECT) {
+        if (G.can_write) G.lcend[G.cpos] = (uint16_t)local;
+        ++G.cpos;
+    } else {
+        wq -= 2u;
+        asm volatile("st.shared.u16 [%0], %1;" :: "r"(wq), "h"((unsigned short)local));
+    }
+}
+
+// fast path: inner if vin <= band, else shell if v < 0; predicated stores and pointer updates, no branches
+template <bool DIRECT>
+__device__ __forceinline__ void record_fast(GroupCtx& G, uint32_t& wp, uint32_t& wq, float vin, float v, float band,
+                                            uint32_t local) {
+    if (DIRECT) {
+        if (vin <= band) record_inner<true>(G, wp, local);
+        else if (v < 0.f) record_shell<true>(G, wq, local);
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pi, ps;\n\t"
+            "setp.le.f32 pi, %2, %3;\n\t"
+            "setp.lt.and.f32 ps, %4, 0f00000000, !pi;\n\t"
+            "@pi st.shared.u16 [%0], %5;\n\t"
+            "@pi add.u32 %0, %0, 2;\n\t"
+            "@ps add.u32 %1, %1, -2;\n\t"
+            "@ps st.shared.u16 [%1], %5;\n\t}"
+            : "+r"(wp), "+r"(wq) : "f"(vin), "f"(band), "f"(v), "h"((unsigned short)local));
     }
 }
 
@@ -198,8 +240,11 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const TravBox& tb, double rk_chi) {
     const uint32_t rowbase = (uint32_t)__cvta_generic_to_shared(&s.hits[lane * kHitStride]);
-    uint32_t wp = rowbase + 2u * G.wpos;          // 32-bit shared-memory address of the lane's next free entry
-    const unsigned long long ax2 = pk2(G.ax, G.ax), ay2 = pk2(G.ay, G.ay), az2 = pk2(G.az, G.az), ra22 = pk2(G.ra2, G.ra2);
+    const uint32_t rowtop = rowbase + 2u * (uint32_t)(kHitCap + kHitSlack);
+    uint32_t wp = rowbase + 2u * G.wpos;          // 32-bit shared-memory addresses: next free inner entry,
+    uint32_t wq = rowtop - 2u * G.cpos;           // lowest shell entry
+    const unsigned long long nkap2 = pk2(-tb.kappa_f, -tb.kappa_f);
+    const unsigned long long ax2 = pk2(G.ax, G.ax), ay2 = pk2(G.ay, G.ay), az2 = pk2(G.az, G.az);
     // software pipeline: the next bucket's candidate (one per lane) is in flight while this one is tested
     double px = 0.0, py = 0.0, pz = 0.0, ph = 0.0;
     if (npend > 0) {
@@ -261,8 +306,8 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             q[0] = 1e18f; q[2] = 1e18f; q[4] = 1e18f; q[6] = 0.f;
         }
         __syncwarp();
-        const uint32_t w0 = wp;
-        const uint32_t nhit0 = G.nhit;
+        const uint32_t w0 = wp, q0 = wq;
+        const uint32_t wpos0 = G.wpos, cpos0 = G.cpos;       // (DIRECT counts entries written in these)
         bool exact = !G.use32;
         if (G.use32) {
             float amin = 3e38f;
@@ -279,19 +324,20 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                     const unsigned long long dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w));
                     const unsigned long long dz = sub2(az2, pk2(c1.x, c1.y));
                     const unsigned long long d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-                    float e0, e1, f0, f1;
-                    upk2(sub2(d2, pk2(c1.z, c1.w)), e0, e1);    // d2 - cutoff_b^2
-                    upk2(sub2(d2, ra22), f0, f1);               // d2 - cutoff_a^2
-                    const float v0 = fminf(e0, f0), v1 = fminf(e1, f1);     // < 0: within the larger cutoff
+                    // M = the larger cutoff^2 of the pair; v = d2 - M (< 0: hit), vin = d2 - kappa M (<= band: inner)
+                    const unsigned long long m2 = pk2(fmaxf(c1.z, G.ra2), fmaxf(c1.w, G.ra2));
+                    float v0, v1, i0, i1;
+                    upk2(sub2(d2, m2), v0, v1);
+                    upk2(fma2(m2, nkap2, d2), i0, i1);
                     amin = fminf(amin, fminf(fabsf(v0), fabsf(v1)));
-                    if (v0 < 0.f) record_hit<DIRECT>(G, wp, id + 2 * u);
-                    if (v1 < 0.f) record_hit<DIRECT>(G, wp, id + 2 * u + 1);
+                    record_fast<DIRECT>(G, wp, wq, i0, v0, band, id + 2 * u);
+                    record_fast<DIRECT>(G, wp, wq, i1, v1, band, id + 2 * u + 1);
                 }
             }
             asm volatile("" ::: "memory");
             // some test of this bucket too close to its cutoff for fp32: the bucket is decided again in fp64
             exact = __any_sync(0xffffffffu, amin <= band);
-            if (exact) { wp = w0; G.nhit = nhit0; }
+            if (exact) { wp = w0; wq = q0; G.wpos = wpos0; G.cpos = cpos0; }
         }
         if (exact) {
             // plain IEEE fp64 test, no FMA contraction: bit-identical to the oracle's decision. One candidate at a
@@ -307,35 +353,51 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                     dz = min_image(dz, tb.L[2], tb.halfL[2], tb.periodic[2]);
                 }
                 const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                if (lt_either(d2, G.rc2q, rc2b)) record_hit<DIRECT>(G, wp, G.ncs + j);
+                if (lt_either(d2, G.rc2q, rc2b)) {
+                    // shell only if surely beyond the inner radius of both (a shell entry wrongly kept inner costs
+                    // time, never correctness)
+                    if (d2 >= tb.kappa * dmax(G.rc2q, rc2b) * (1.0 + 1e-9)) record_shell<DIRECT>(G, wq, G.ncs + j);
+                    else record_inner<DIRECT>(G, wp, G.ncs + j);
+                }
             }
             asm volatile("" ::: "memory");
         }
         if (!DIRECT) {
-            G.nhit += (wp - w0) >> 1;
+            G.nhit += ((wp - w0) + (q0 - wq)) >> 1;
+            G.nin += (wp - w0) >> 1;
             G.wpos = (wp - rowbase) >> 1;
-            // A row has room for one more bucket only up to kHitCap: when some lane is beyond it, every lane moves
-            // its row to its part of the warp's global scratch (the list order is kept: spilled part, then the row);
-            // when that is full too the group is counted on and walked a second time writing directly.
-            if (__any_sync(0xffffffffu, G.wpos > (uint32_t)kHitCap)) {
-                if (!G.hard_overflow && __all_sync(0xffffffffu, G.nspill + G.wpos <= (uint32_t)kSpillCap)) {
-                    // the warp moves one row at a time (coalesced 16-bit stores; lane by lane the stores of a row
-                    // fell into 32 different sectors per instruction)
+            G.cpos = (rowtop - wq) >> 1;
+            // A row keeps room for one more bucket only while it holds at most kHitCap entries: when some lane is beyond
+            // that, every lane moves its row to its part of the warp's global scratch (same two-ended layout; the
+            // order of the inner entries is kept: spilled part, then the row); when that is full too the group is
+            // counted on and walked a second time writing directly.
+            if (__any_sync(0xffffffffu, G.wpos + G.cpos > (uint32_t)kHitCap)) {
+                if (!G.hard_overflow &&
+                    __all_sync(0xffffffffu, G.nspill + G.wpos + G.cspill + G.cpos <= (uint32_t)kSpillCap)) {
+                    // the warp moves one row at a time (coalesced 16-bit stores)
                     __syncwarp();
                     for (uint32_t p = 0; p < 32u; ++p) {
                         const uint32_t wn = __shfl_sync(0xffffffffu, G.wpos, p), ns = __shfl_sync(0xffffffffu, G.nspill, p);
+                        const uint32_t cn = __shfl_sync(0xffffffffu, G.cpos, p), cs = __shfl_sync(0xffffffffu, G.cspill, p);
                         uint16_t* dst = G.hspill + (size_t)p * kSpillCap + ns;
                         for (uint32_t k = lane; k < wn; k += 32) dst[k] = s.hits[p * kHitStride + k];
+                        uint16_t* dsc = G.hspill + (size_t)p * kSpillCap + (kSpillCap - cs - cn);
+                        for (uint32_t k = lane; k < cn; k += 32) dsc[k] = s.hits[p * kHitStride + (kHitCap + kHitSlack - cn) + k];
                     }
                     __syncwarp();
                     G.nspill += G.wpos;
-                    G.wpos = 0u;
+                    G.cspill += G.cpos;
                 } else {
-                    G.hard_overflow = true;
-                    if (G.wpos > (uint32_t)kHitCap) G.wpos = (uint32_t)kHitCap;
+                    G.hard_overflow = true;       // the rows' content no longer matters, only the counts
                 }
-                wp = rowbase + 2u * G.wpos;
+                G.wpos = 0u;
+                G.cpos = 0u;
+                wp = rowbase;
+                wq = rowtop;
             }
+        } else {
+            G.nhit = G.wpos + G.cpos;
+            G.nin = G.wpos;
         }
         G.ncs += nk;
     }
@@ -426,7 +488,7 @@ __device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, uns
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.nspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
+    G.nhit = 0u; G.nin = 0u; G.wpos = 0u; G.cpos = 0u; G.nspill = 0u; G.cspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
     int nb = 0;
     __syncwarp();
     for (int base = 0; base < nu; base += 32) {
@@ -456,7 +518,7 @@ __device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
-    G.nhit = 0u; G.wpos = 0u; G.nspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
+    G.nhit = 0u; G.nin = 0u; G.wpos = 0u; G.cpos = 0u; G.nspill = 0u; G.cspill = 0u; G.hard_overflow = false; G.ncs = 0u; G.anywrap = false;
     int sp = 1, nb = 0;
     __syncwarp();
     if (lane == 0) s.stack[0] = (N == 1) ? kLeafBit : 0u;
@@ -613,8 +675,9 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             G.ax = (float)((G.xq - G.cx) * G.sc); G.ay = (float)((G.yq - G.cy) * G.sc); G.az = (float)((G.zq - G.cz) * G.sc);
             G.ra2 = (float)(G.rc2q * G.sc * G.sc);
             G.rca = (float)(rk_chi * hq * G.sc) * 1.000001f;
+            G.kin_a = tb.kappa_f * G.ra2;
         }
-        if (!qv) { G.xq = -1e300; G.rc2q = 0.0; G.ax = G.ay = G.az = -1e18f; G.ra2 = 0.f; G.rca = 0.f; }   // lanes without a particle can never hit
+        if (!qv) { G.xq = -1e300; G.rc2q = 0.0; G.ax = G.ay = G.az = -1e18f; G.ra2 = 0.f; G.rca = 0.f; G.kin_a = 0.f; }   // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
         G.hspill = hit_row;
 
@@ -622,8 +685,10 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         else walk<false>(s, G, lane, lt, N, x, y, z, h, nodes, tb, rk_chi);
 
         // ---- allocate from the exact counts: lists and candidate slots ----
-        // every particle's list starts at a multiple of eight entries (16 B), so that rows are copied out as uint4
-        const uint32_t nhit = qv ? G.nhit : 0u, nhit4 = (nhit + 7u) & ~7u;
+        // A particle's list: its inner entries, then its shell entries (any order); every list starts at a multiple of
+        // eight entries (16 B), so that rows are copied out as uint4
+        const uint32_t nhit = qv ? G.nhit : 0u, nin = qv ? G.nin : 0u;
+        const uint32_t nhit4 = (nhit + 7u) & ~7u;
         const uint32_t nc = G.ncs, nc4 = (nc + 3u) & ~3u;
         uint32_t incl = nhit4;
 #pragma unroll
@@ -632,11 +697,13 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             if (lane >= (unsigned)o) incl += t;
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, 31), total_exact = __reduce_add_sync(0xffffffffu, nhit);
+        const uint32_t total_inner = __reduce_add_sync(0xffffffffu, nin);
         unsigned long long lbase = 0, bbase = 0;
         if (lane == 0) {
             lbase = atomicAdd(&sc->list_cursor, (unsigned long long)((total + 7u) & ~7u));
             bbase = atomicAdd(&sc->cslot_cursor, (unsigned long long)nc4);
             atomicAdd(&sc->n_neigh, (unsigned long long)total_exact);
+            atomicAdd(&sc->n_inner, (unsigned long long)total_inner);
         }
         lbase = __shfl_sync(0xffffffffu, lbase, 0);
         bbase = __shfl_sync(0xffffffffu, bbase, 0);
@@ -645,6 +712,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
         const uint64_t my_start = lbase + (incl - nhit4);
         if (qv) {
             out.cnt[a] = nhit;
+            out.cnt_in[a] = nin;
             out.lstart[a] = my_start;
         }
         if (fits) {
@@ -662,30 +730,37 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                     uint4* dst = reinterpret_cast<uint4*>(out.cslot + bbase);
                     for (uint32_t j = lane; j < (nc4 >> 2); j += 32) dst[j] = src[j];
                 }
-                // lists: the warp copies one particle's buffered list at a time (coalesced)
-                const bool spilled = __any_sync(0xffffffffu, G.nspill != 0u);
+                const bool spilled = __any_sync(0xffffffffu, (G.nspill | G.cspill) != 0u);
                 if (!spilled) {
-                    // every lane copies its own row, 16 bytes per store (the up to seven entries of padding are never
-                    // read): a store instruction touches 32 lists, half a sector each, and consecutive instructions
-                    // fill the sectors in L2; a row-by-row copy by the whole warp is coalesced but costs 30 times the
-                    // instructions
-                    const uint4* src = reinterpret_cast<const uint4*>(&s.hits[lane * kHitStride]);
+                    // every lane copies its own row, 16 bytes per store: a store instruction touches 32 lists, half a
+                    // sector each, and consecutive instructions fill the sectors in L2; a row-by-row copy by the whole
+                    // warp is coalesced but costs 30 times the instructions
+                    // (the lane first moves its shell entries from the row top down to the end of its inner entries)
+                    uint16_t* rowp = &s.hits[lane * kHitStride];
+                    for (uint32_t k = 0; k < nhit - nin; ++k) rowp[nin + k] = rowp[(kHitCap + kHitSlack) - (nhit - nin) + k];
+                    const uint4* src = reinterpret_cast<const uint4*>(rowp);
                     uint4* dst = reinterpret_cast<uint4*>(out.lists + my_start);
                     for (uint32_t k = 0; k < (nhit4 >> 3); ++k) dst[k] = src[k];
                 } else {
+                    // the warp copies one particle's list at a time: spilled inner part, inner part of the row, then
+                    // the shell entries of the row and of the scratch (any order)
                     for (uint32_t p = 0; p < nq; ++p) {
-                        const uint32_t np = __shfl_sync(0xffffffffu, nhit, p);
-                        uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - ((np + 7u) & ~7u));
-                        const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p);
+                        const uint32_t np8 = __shfl_sync(0xffffffffu, nhit4, p);
+                        uint64_t sp0 = lbase + (__shfl_sync(0xffffffffu, incl, p) - np8);
+                        const uint32_t ns = __shfl_sync(0xffffffffu, G.nspill, p), wn = __shfl_sync(0xffffffffu, G.wpos, p);
+                        const uint32_t cs = __shfl_sync(0xffffffffu, G.cspill, p), cn = __shfl_sync(0xffffffffu, G.cpos, p);
                         const uint16_t* src = hit_row + (size_t)p * kSpillCap;
                         for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
-                        sp0 += ns;
-                        for (uint32_t k = lane; k < np - ns; k += 32) out.lists[sp0 + k] = s.hits[p * kHitStride + k];
+                        for (uint32_t k = lane; k < wn; k += 32) out.lists[sp0 + ns + k] = s.hits[p * kHitStride + k];
+                        const uint64_t se = sp0 + ns + wn;
+                        for (uint32_t k = lane; k < cn; k += 32) out.lists[se + k] = s.hits[p * kHitStride + (kHitCap + kHitSlack - cn) + k];
+                        for (uint32_t k = lane; k < cs; k += 32) out.lists[se + cn + k] = src[kSpillCap - cs + k];
                     }
                 }
             } else {
                 // fallback: second walk writing directly at the now-known positions
                 G.lptr = out.lists + my_start;
+                G.lcend = G.lptr + nin;
                 G.cptr = out.cslot + bbase;
                 G.can_write = true;
                 if (nu >= 0) refine<true>(s, G, nu, lane, lt, x, y, z, h, nodes, tb, rk_chi);
@@ -712,7 +787,7 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
 __global__ void k_trav_reset(uint32_t* work_counter, DevScalars* sc) {
     *work_counter = 0u;
     sc->nbr_min = 0xffffffffu; sc->nbr_max = 0u;
-    sc->list_cursor = 0ull; sc->cslot_cursor = 0ull; sc->n_neigh = 0ull;
+    sc->list_cursor = 0ull; sc->cslot_cursor = 0ull; sc->n_neigh = 0ull; sc->n_inner = 0ull;
     sc->nc_max = 0u; sc->n_cand_overflow = 0u; sc->n_chunks_shared = 0u; sc->n_chunks_overflow = 0u; sc->n_fallback = 0u;
 }
 
@@ -734,9 +809,11 @@ int launch_traverse(sph_ctx* c) {
     tb.gg_pad = 1e-14 * Lmax;
     tb.gmax = (uint32_t)c->p.group_max;
     tb.lscan = c->p.leaf_reduction >= 1 ? c->lscan : nullptr;
+    tb.kappa = fmin(1.0, ((1.0 + kShellEps) / c->p.chi) * ((1.0 + kShellEps) / c->p.chi));
+    tb.kappa_f = (float)tb.kappa;
     const double rk_chi = kern_radius(c->p.kernel) * c->p.chi;
     TravOut out;
-    out.cnt = c->cnt; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
+    out.cnt = c->cnt; out.cnt_in = c->cnt_in; out.lstart = c->lstart; out.lists = c->lists; out.list_cap = c->list_cap;
     out.cslot = c->cslot; out.cslot_cap = c->cslot_cap; out.scratch = c->trav_scratch; out.hit_scratch = c->trav_hit_scratch; out.ginfo = c->ginfo; out.ginfo_cap = c->ginfo_cap;
     uint32_t* wc = c->sort_counters + 8;   // spare counter word
     k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc);
@@ -762,6 +839,7 @@ __global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t*
                                                       const GroupRec* __restrict__ ginfo,
                                                       const uint32_t* __restrict__ cslot,
                                                       const uint32_t* __restrict__ cnt,
+                                                      const uint32_t* __restrict__ cnt_in,
                                                       const uint64_t* __restrict__ lstart,
                                                       const uint16_t* __restrict__ lists,
                                                       const uint64_t* __restrict__ offs, uint32_t* __restrict__ idx,
@@ -779,7 +857,7 @@ __global__ void __launch_bounds__(256) k_cache_to_csr(int64_t N, const uint32_t*
 
 // lists of the sorted slots [first, first + count) into idx_out, which starts at the first slot's list
 int launch_cache_to_csr(sph_ctx* c, uint32_t* idx_out, int64_t first, int64_t count) {
-    k_cache_to_csr<<<div_up(count, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->cslot, c->cnt, c->lstart,
+    k_cache_to_csr<<<div_up(count, 256), 256, 0, c->stream>>>(c->N, c->gscan, c->ginfo, c->cslot, c->cnt, c->cnt_in, c->lstart,
                                                               c->lists, c->offs, idx_out, first, count);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());

@@ -13,7 +13,7 @@ constexpr uint64_t kSFlagAgg = 1ull << 62, kSFlagIncl = 2ull << 62, kSValMask = 
 template <typename OutT>
 __global__ void __launch_bounds__(kScanThreads) k_scan(const uint32_t* __restrict__ in, OutT* __restrict__ out, int64_t n,
                                                        volatile uint64_t* status, uint32_t* counter,
-                                                       unsigned long long* total_out) {
+                                                       unsigned long long* total_out, uint32_t* fill, DevScalars* sc) {
     __shared__ uint64_t wsum[kScanThreads / 32];
     __shared__ uint64_t s_excl;
     __shared__ uint32_t s_tile;
@@ -77,25 +77,30 @@ __global__ void __launch_bounds__(kScanThreads) k_scan(const uint32_t* __restric
     uint64_t run = s_excl + wbase + inc - tsum;
 #pragma unroll
     for (int i = 0; i < kScanItems; ++i) {
-        if (base + i < n) out[base + i] = (OutT)run;
+        if (base + i < n) {
+            out[base + i] = (OutT)run;
+            if (fill && v[i]) fill[run] = (uint32_t)(base + i);      // stream compaction of the flagged positions
+        }
         run += v[i];
     }
     // the tile holding item n-1 also writes the total
     if (base <= n - 1 && n - 1 < base + kScanItems) {
         out[n] = (OutT)run;
         if (total_out) *total_out = run;
+        if (fill) { fill[run] = (uint32_t)n; sc->n_groups = (unsigned int)run; }
     }
 }
 
 int scan_scratch_tiles(int64_t N) { return (int)((N + 1 + kScanTile - 1) / kScanTile) + 1; }
 
 template <typename OutT>
-static int scan_impl(sph_ctx* c, const uint32_t* in, OutT* out, int64_t n, unsigned long long* total_out) {
+static int scan_impl(sph_ctx* c, const uint32_t* in, OutT* out, int64_t n, unsigned long long* total_out,
+                     uint32_t* fill = nullptr) {
     if (n <= 0) return SPH_OK;
     int64_t tiles = (n + kScanTile - 1) / kScanTile;
     SPH_CUDA(c, cudaMemsetAsync(c->scan_status, 0, (size_t)tiles * sizeof(uint64_t), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(c->scan_counter, 0, sizeof(uint32_t), c->stream));
-    k_scan<OutT><<<(unsigned)tiles, kScanThreads, 0, c->stream>>>(in, out, n, c->scan_status, c->scan_counter, total_out);
+    k_scan<OutT><<<(unsigned)tiles, kScanThreads, 0, c->stream>>>(in, out, n, c->scan_status, c->scan_counter, total_out, fill, c->d_sc);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -103,6 +108,11 @@ static int scan_impl(sph_ctx* c, const uint32_t* in, OutT* out, int64_t n, unsig
 
 int launch_scan_u32_u64(sph_ctx* c, const uint32_t* in, uint64_t* out, int64_t n, unsigned long long* total_out) {
     return scan_impl<uint64_t>(c, in, (uint64_t*)out, n, total_out);
+}
+// leaf groups: exclusive scan of the group-start flags (0 / 1) and, in the same pass, grp_lo[g] = first slot of group g,
+// grp_lo[n_groups] = n and the group count (tree.cu)
+int launch_scan_groups(sph_ctx* c, const uint32_t* gflag, uint32_t* gscan, uint32_t* grp_lo, int64_t n) {
+    return scan_impl<uint32_t>(c, gflag, gscan, n, nullptr, grp_lo);
 }
 __global__ void k_store_u32(const unsigned long long* src, unsigned int* dst) { *dst = (unsigned int)*src; }
 int launch_scan_u32_u32(sph_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, unsigned int* total_out) {

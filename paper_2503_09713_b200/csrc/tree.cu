@@ -95,19 +95,6 @@ __global__ void __launch_bounds__(256) k_karras(int64_t N64, const uint64_t* __r
     }
 }
 
-__global__ void __launch_bounds__(256) k_group_fill(int64_t N, const uint32_t* __restrict__ gflag,
-                                                    const uint32_t* __restrict__ gscan, uint32_t* __restrict__ grp_lo,
-                                                    DevScalars* sc) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    if (gflag[i]) grp_lo[gscan[i]] = (uint32_t)i;
-    if (i == N - 1) {
-        uint32_t ng = gscan[N];
-        grp_lo[ng] = (uint32_t)N;
-        sc->n_groups = ng;
-    }
-}
-
 // a3b: bottom-up boxes. A thread carrying a finished child box up the tree announces itself at the parent with an
 // atomic flag; the second arrival merges both children and goes on. Sibling records are read with L2 loads (ld.cg)
 // issued after the flag atomic has returned, so only the release side (record written -> fence -> flag) needs a fence.
@@ -260,9 +247,7 @@ int launch_tree(sph_ctx* c) {
         k_single_group<<<1, 1, 0, c->stream>>>(c->gflag);
         c->launches++;
     }
-    SPH_TRY(launch_scan_u32_u32(c, c->gflag, c->gscan, N, nullptr));
-    k_group_fill<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->gflag, c->gscan, c->grp_lo, c->d_sc);
-    c->launches++;
+    SPH_TRY(launch_scan_groups(c, c->gflag, c->gscan, c->grp_lo, N));      // scan + grp_lo + group count in one pass
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }
