@@ -592,14 +592,19 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
     const double* __restrict__ h, const NodeRec* __restrict__ nodes, const uint32_t* __restrict__ grp_lo,
     TravBox tb, double rk_chi, TravOut out, uint32_t* work_counter, DevScalars* sc, uint32_t chunk) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    TravWarpSmem& s = reinterpret_cast<TravWarpSmem*>(smem_raw)[threadIdx.x >> 5];
+    // (values that every bucket of every group needs are passed through empty asm statements: the compiler otherwise
+    // recomputes them inside the bucket loop -- a tenth of the kernel's instructions -- although registers are free)
+    unsigned soff = (threadIdx.x >> 5) * (unsigned)sizeof(TravWarpSmem);
+    asm volatile("" : "+r"(soff));
+    TravWarpSmem& s = *reinterpret_cast<TravWarpSmem*>(smem_raw + soff);
     const unsigned lane = lane_id();
     const unsigned lt = lanemask_lt();
     const uint32_t n_groups = sc->n_groups;
     const double reach_max = rk_chi * sc->h_max * 1.001;   // the largest cutoff radius of any particle (k_hmax ran before)
     unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u;
     uint16_t* const hit_row = out.hit_scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * (32 * kSpillCap);
-    uint32_t* const scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
+    uint32_t* scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
+    asm volatile("" : "+l"(scr_row));
 
     for (;;) {
         uint32_t g0 = 0;
@@ -676,6 +681,8 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
             G.ra2 = (float)(G.rc2q * G.sc * G.sc);
             G.rca = (float)(rk_chi * hq * G.sc) * 1.000001f;
             G.kin_a = tb.kappa_f * G.ra2;
+            asm volatile("" : "+f"(G.ex), "+f"(G.ey), "+f"(G.ez), "+f"(G.twoA), "+f"(G.rcg), "+f"(G.rc2g_f));
+            asm volatile("" : "+d"(G.sc), "+d"(G.ksc), "+d"(G.cx), "+d"(G.cy), "+d"(G.cz));
         }
         if (!qv) { G.xq = -1e300; G.rc2q = 0.0; G.ax = G.ay = G.az = -1e18f; G.ra2 = 0.f; G.rca = 0.f; G.kin_a = 0.f; }   // lanes without a particle can never hit
         G.lptr = nullptr; G.cptr = scr_row; G.can_write = false;
