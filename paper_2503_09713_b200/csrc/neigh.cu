@@ -29,7 +29,7 @@
 //     both are written out coalesced once the group is complete; space comes from two bump allocators (count ->
 //     allocate -> fill per group; the host re-runs the pass with larger pools if one overflowed). A group whose
 //     lists outgrow the shared-memory rows spills them to a per-warp scratch in global memory; beyond that (lists
-//     longer than kSpillCap + kHitCap, more than kScrCap candidates) it allocates from its exact counts and walks a
+//     longer than kSpillCap + the row capacity, more than kScrCap candidates) it allocates from its exact counts and walks a
 //     second time writing directly.
 #include <stdlib.h>
 
@@ -41,11 +41,10 @@ constexpr int kTravWarps = 8;            // warps per block
 constexpr int kStackCap = 512;           // stack entries per warp
 constexpr int kStackSlack = 192;         // above kStackCap - kStackSlack the warp pops one node at a time (pure DFS)
 constexpr int kPendCap = 64;             // candidate buckets buffered before stage 2 runs
-constexpr int kHitCap = 112;             // buffered hits per lane
+constexpr int kHitCapR2 = 112, kHitCapR3 = 224;   // buffered hits per lane: kernels of radius 2; M5 / M6
+constexpr int kTravWarpsR3 = 5;          // warps per block with the larger rows
 constexpr int kHitSlack = 32;            // room for one more bucket beyond kHitCap (overflow is checked per bucket)
-constexpr int kHitStride = kHitCap + kHitSlack + 8;   // in u16: 304 B per lane row, 16-byte aligned (copied out as uint4; 76 words
-                                                      // per row also spreads the 32 rows' LDS.128 over all banks)
-static_assert(kHitStride % 8 == 0, "hit rows are copied as 16-byte words");
+static_assert((kHitCapR2 + kHitSlack + 8) % 8 == 0 && (kHitCapR3 + kHitSlack + 8) % 8 == 0, "hit rows are copied as 16-byte words");
 constexpr int kShare = 4;               // consecutive groups that share one tree walk
 constexpr int kUbCap = 192;             // bucket nodes collected by the shared walk
 constexpr int kSpillCap = 512;            // hits per lane that can spill from the shared-memory row to the warp's global scratch
@@ -64,7 +63,11 @@ struct TravBox {
                                          // inside one reduced leaf: lscan[hi + 1] == lscan[lo + 1]
 };
 
-struct TravWarpSmem {
+// HC = hit-row capacity in entries (lists of a group's particles are buffered here): 112 for the kernels of radius 2
+// (about 81 neighbours at h_fact 1.2), 224 for M5 / M6 (about 157), which then run five warps per CTA
+template <int HC>
+struct TravWarpSmemT {
+    static constexpr int kCap = HC, kStride = HC + kHitSlack + 8;   // in u16; rows 16-byte aligned (copied out as uint4)
     uint32_t stack[kStackCap];
     uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
     float prc[kPendCap];                      // their reach R_kern chi hmax_node in the group's scaled units, rounded up
@@ -72,7 +75,7 @@ struct TravWarpSmem {
                                               // scaled fp32 coordinates relative to the group's centre, r = cutoff^2
     uint32_t cslotb[kGroup];                  // their sorted slots (exact path)
     uint32_t ub[kUbCap];                      // bucket nodes within reach of the kShare groups' common box
-    __align__(16) uint16_t hits[32 * kHitStride];
+    __align__(16) uint16_t hits[32 * kStride];
 };
 
 struct TravOut {
@@ -234,13 +237,13 @@ __device__ __forceinline__ void record_fast(GroupCtx& G, uint32_t& wp, uint32_t&
 // rcm' = the larger of the query's and the bucket's reach (true hit: d <= rcm'; true miss: d2 - err(d) is increasing in
 // d beyond rcm', or E > rcm' / sqrt(3) and 12 E^2 covers it). So |v_f| > B implies sign(v_f) = sign(v), and sign(v) is
 // the fp64 decision because that differs from the real-number one only within 1e-15 relative of the cutoff.
-template <bool DIRECT>
-__device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, unsigned lane, unsigned lt,
+template <bool DIRECT, class S>
+__device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned lane, unsigned lt,
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const TravBox& tb, double rk_chi) {
-    const uint32_t rowbase = (uint32_t)__cvta_generic_to_shared(&s.hits[lane * kHitStride]);
-    const uint32_t rowtop = rowbase + 2u * (uint32_t)(kHitCap + kHitSlack);
+    const uint32_t rowbase = (uint32_t)__cvta_generic_to_shared(&s.hits[lane * S::kStride]);
+    const uint32_t rowtop = rowbase + 2u * (uint32_t)(S::kCap + kHitSlack);
     uint32_t wp = rowbase + 2u * G.wpos;          // 32-bit shared-memory addresses: next free inner entry,
     uint32_t wq = rowtop - 2u * G.cpos;           // lowest shell entry
     const unsigned long long nkap2 = pk2(-tb.kappa_f, -tb.kappa_f);
@@ -367,11 +370,11 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
             G.nin += (wp - w0) >> 1;
             G.wpos = (wp - rowbase) >> 1;
             G.cpos = (rowtop - wq) >> 1;
-            // A row keeps room for one more bucket only while it holds at most kHitCap entries: when some lane is beyond
+            // A row keeps room for one more bucket only while it holds at most HC entries: when some lane is beyond
             // that, every lane moves its row to its part of the warp's global scratch (same two-ended layout; the
             // order of the inner entries is kept: spilled part, then the row); when that is full too the group is
             // counted on and walked a second time writing directly.
-            if (__any_sync(0xffffffffu, G.wpos + G.cpos > (uint32_t)kHitCap)) {
+            if (__any_sync(0xffffffffu, G.wpos + G.cpos > (uint32_t)S::kCap)) {
                 if (!G.hard_overflow &&
                     __all_sync(0xffffffffu, G.nspill + G.wpos + G.cspill + G.cpos <= (uint32_t)kSpillCap)) {
                     // the warp moves one row at a time (coalesced 16-bit stores)
@@ -380,9 +383,9 @@ __device__ __forceinline__ void stage2(TravWarpSmem& s, GroupCtx& G, int npend, 
                         const uint32_t wn = __shfl_sync(0xffffffffu, G.wpos, p), ns = __shfl_sync(0xffffffffu, G.nspill, p);
                         const uint32_t cn = __shfl_sync(0xffffffffu, G.cpos, p), cs = __shfl_sync(0xffffffffu, G.cspill, p);
                         uint16_t* dst = G.hspill + (size_t)p * kSpillCap + ns;
-                        for (uint32_t k = lane; k < wn; k += 32) dst[k] = s.hits[p * kHitStride + k];
+                        for (uint32_t k = lane; k < wn; k += 32) dst[k] = s.hits[p * S::kStride + k];
                         uint16_t* dsc = G.hspill + (size_t)p * kSpillCap + (kSpillCap - cs - cn);
-                        for (uint32_t k = lane; k < cn; k += 32) dsc[k] = s.hits[p * kHitStride + (kHitCap + kHitSlack - cn) + k];
+                        for (uint32_t k = lane; k < cn; k += 32) dsc[k] = s.hits[p * S::kStride + (S::kCap + kHitSlack - cn) + k];
                     }
                     __syncwarp();
                     G.nspill += G.wpos;
@@ -448,7 +451,8 @@ __device__ __forceinline__ NodeHit node_test(uint32_t e, const GroupCtx& G, cons
 // particles) within reach of U into s.ub. Every bucket a member group needs is among them: the group's box lies
 // inside U and its hmax is not larger, every operation of the test is monotone, so a node that passes the group's
 // test passes U's, and so do all its ancestors. Returns the number of buckets, or -1 if s.ub overflowed.
-__device__ __forceinline__ int walk_collect(TravWarpSmem& s, const GroupCtx& U, unsigned lane, unsigned lt, int64_t N,
+template <class S>
+__device__ __forceinline__ int walk_collect(S& s, const GroupCtx& U, unsigned lane, unsigned lt, int64_t N,
                                             const double* __restrict__ x, const double* __restrict__ y,
                                             const double* __restrict__ z, const double* __restrict__ h,
                                             const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
@@ -483,8 +487,8 @@ __device__ __forceinline__ int walk_collect(TravWarpSmem& s, const GroupCtx& U, 
 }
 
 // One group's buckets out of the collected ones (the same test with the group's own box), then stage 2.
-template <bool DIRECT>
-__device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, unsigned lane, unsigned lt,
+template <bool DIRECT, class S>
+__device__ __forceinline__ void refine(S& s, GroupCtx& G, int nu, unsigned lane, unsigned lt,
                                        const double* __restrict__ x, const double* __restrict__ y,
                                        const double* __restrict__ z, const double* __restrict__ h,
                                        const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
@@ -513,8 +517,8 @@ __device__ __forceinline__ void refine(TravWarpSmem& s, GroupCtx& G, int nu, uns
 }
 
 // one complete walk of the tree for the group described by G (used when the shared walk overflowed s.ub)
-template <bool DIRECT>
-__device__ __forceinline__ void walk(TravWarpSmem& s, GroupCtx& G, unsigned lane, unsigned lt, int64_t N,
+template <bool DIRECT, class S>
+__device__ __forceinline__ void walk(S& s, GroupCtx& G, unsigned lane, unsigned lt, int64_t N,
                                      const double* __restrict__ x, const double* __restrict__ y,
                                      const double* __restrict__ z, const double* __restrict__ h,
                                      const NodeRec* __restrict__ nodes, const TravBox& tb, double rk_chi) {
@@ -587,23 +591,24 @@ __device__ __forceinline__ uint32_t warp_max_u32(uint32_t v) {
     return v;
 }
 
-__global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
+template <int HC, int W>
+__global__ void __launch_bounds__(W * 32, 2) k_traverse(
     int64_t N, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
     const double* __restrict__ h, const NodeRec* __restrict__ nodes, const uint32_t* __restrict__ grp_lo,
     TravBox tb, double rk_chi, TravOut out, uint32_t* work_counter, DevScalars* sc, uint32_t chunk) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // (values that every bucket of every group needs are passed through empty asm statements: the compiler otherwise
     // recomputes them inside the bucket loop -- a tenth of the kernel's instructions -- although registers are free)
-    unsigned soff = (threadIdx.x >> 5) * (unsigned)sizeof(TravWarpSmem);
+    unsigned soff = (threadIdx.x >> 5) * (unsigned)sizeof(TravWarpSmemT<HC>);
     asm volatile("" : "+r"(soff));
-    TravWarpSmem& s = *reinterpret_cast<TravWarpSmem*>(smem_raw + soff);
+    TravWarpSmemT<HC>& s = *reinterpret_cast<TravWarpSmemT<HC>*>(smem_raw + soff);
     const unsigned lane = lane_id();
     const unsigned lt = lanemask_lt();
     const uint32_t n_groups = sc->n_groups;
     const double reach_max = rk_chi * sc->h_max * 1.001;   // the largest cutoff radius of any particle (k_hmax ran before)
     unsigned mn = 0xffffffffu, mx = 0u, ncmax = 0u;
-    uint16_t* const hit_row = out.hit_scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * (32 * kSpillCap);
-    uint32_t* scr_row = out.scratch + ((size_t)blockIdx.x * kTravWarps + (threadIdx.x >> 5)) * kScrCap;
+    uint16_t* const hit_row = out.hit_scratch + ((size_t)blockIdx.x * W + (threadIdx.x >> 5)) * (32 * kSpillCap);
+    uint32_t* scr_row = out.scratch + ((size_t)blockIdx.x * W + (threadIdx.x >> 5)) * kScrCap;
     asm volatile("" : "+l"(scr_row));
 
     for (;;) {
@@ -743,8 +748,8 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                     // sector each, and consecutive instructions fill the sectors in L2; a row-by-row copy by the whole
                     // warp is coalesced but costs 30 times the instructions
                     // (the lane first moves its shell entries from the row top down to the end of its inner entries)
-                    uint16_t* rowp = &s.hits[lane * kHitStride];
-                    for (uint32_t k = 0; k < nhit - nin; ++k) rowp[nin + k] = rowp[(kHitCap + kHitSlack) - (nhit - nin) + k];
+                    uint16_t* rowp = &s.hits[lane * (HC + kHitSlack + 8)];
+                    for (uint32_t k = 0; k < nhit - nin; ++k) rowp[nin + k] = rowp[(HC + kHitSlack) - (nhit - nin) + k];
                     const uint4* src = reinterpret_cast<const uint4*>(rowp);
                     uint4* dst = reinterpret_cast<uint4*>(out.lists + my_start);
                     for (uint32_t k = 0; k < (nhit4 >> 3); ++k) dst[k] = src[k];
@@ -758,9 +763,9 @@ __global__ void __launch_bounds__(kTravWarps * 32, 2) k_traverse(
                         const uint32_t cs = __shfl_sync(0xffffffffu, G.cspill, p), cn = __shfl_sync(0xffffffffu, G.cpos, p);
                         const uint16_t* src = hit_row + (size_t)p * kSpillCap;
                         for (uint32_t k = lane; k < ns; k += 32) out.lists[sp0 + k] = src[k];
-                        for (uint32_t k = lane; k < wn; k += 32) out.lists[sp0 + ns + k] = s.hits[p * kHitStride + k];
+                        for (uint32_t k = lane; k < wn; k += 32) out.lists[sp0 + ns + k] = s.hits[p * (HC + kHitSlack + 8) + k];
                         const uint64_t se = sp0 + ns + wn;
-                        for (uint32_t k = lane; k < cn; k += 32) out.lists[se + k] = s.hits[p * kHitStride + (kHitCap + kHitSlack - cn) + k];
+                        for (uint32_t k = lane; k < cn; k += 32) out.lists[se + k] = s.hits[p * (HC + kHitSlack + 8) + (HC + kHitSlack - cn) + k];
                         for (uint32_t k = lane; k < cs; k += 32) out.lists[se + cn + k] = src[kSpillCap - cs + k];
                     }
                 }
@@ -803,8 +808,12 @@ size_t trav_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * kScrCa
 size_t trav_hit_scratch_entries() { return (size_t)kTravBlocks * kTravWarps * 32 * kSpillCap; }
 
 int launch_traverse(sph_ctx* c) {
-    const int smem = (int)sizeof(TravWarpSmem) * kTravWarps;
-    SPH_CUDA(c, cudaFuncSetAttribute(k_traverse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));   // per device: every launch
+    // hit rows sized for the kernel's neighbour count: radius 2 -> 112 entries, 8 warps per CTA; M5 / M6 -> 224, 5 warps
+    const bool wide = kern_radius(c->p.kernel) > 2.0;
+    const int W = wide ? kTravWarpsR3 : kTravWarps;
+    const int smem = wide ? (int)sizeof(TravWarpSmemT<kHitCapR3>) * kTravWarpsR3 : (int)sizeof(TravWarpSmemT<kHitCapR2>) * kTravWarps;
+    if (wide) SPH_CUDA(c, cudaFuncSetAttribute(k_traverse<kHitCapR3, kTravWarpsR3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    else SPH_CUDA(c, cudaFuncSetAttribute(k_traverse<kHitCapR2, kTravWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));   // per device: every launch
     TravBox tb;
     double Lmax = 0.0;
     for (int k = 0; k < 3; ++k) {
@@ -826,16 +835,20 @@ int launch_traverse(sph_ctx* c) {
     k_trav_reset<<<1, 1, 0, c->stream>>>(wc, c->d_sc);
     // persistent grid: two CTAs per SM (shared-memory bound), work handed out through an atomic counter
     const int64_t warps_needed = (c->N + 31) / 32;
-    unsigned blocks = (unsigned)min((int64_t)kTravBlocks, (warps_needed + kTravWarps - 1) / kTravWarps);
+    unsigned blocks = (unsigned)min((int64_t)kTravBlocks, (warps_needed + W - 1) / W);
     if (blocks == 0) blocks = 1;
     // Shared walks (kShare consecutive groups per warp) pay when there are many groups per warp and the groups of a
     // chunk are alike; api.cu switches them off for good if the last pass shared too few chunks.
     // SPH_FORCE_SHARE=1 (tests) forces shared walks whatever the problem size.
     const bool force = getenv("SPH_FORCE_SHARE") != nullptr;
-    const uint32_t chunk = (force || (!c->share_disabled && c->n_groups >= (int64_t)32 * kTravBlocks * kTravWarps)) ? kShare : 1u;
+    const uint32_t chunk = (force || (!c->share_disabled && c->n_groups >= (int64_t)32 * kTravBlocks * W)) ? kShare : 1u;
     c->last_chunk = chunk;
-    k_traverse<<<blocks, kTravWarps * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
-                                                             c->grp_lo, tb, rk_chi, out, wc, c->d_sc, chunk);
+    if (wide)
+        k_traverse<kHitCapR3, kTravWarpsR3><<<blocks, W * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
+                                                                              c->grp_lo, tb, rk_chi, out, wc, c->d_sc, chunk);
+    else
+        k_traverse<kHitCapR2, kTravWarps><<<blocks, W * 32, smem, c->stream>>>(c->N, c->cur.x, c->cur.y, c->cur.z, c->cur.h, c->nodes,
+                                                                            c->grp_lo, tb, rk_chi, out, wc, c->d_sc, chunk);
     c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
