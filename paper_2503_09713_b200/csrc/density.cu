@@ -10,6 +10,8 @@
 // kept in registers for every Newton sweep (r does not depend on h): a sweep costs only the kernel evaluation and
 // two three-step octet reductions. Lists longer than 96 entries re-gather the excess from shared memory per
 // sweep. Groups whose buckets cannot wrap around a periodic axis use plain differences. No global gathers remain.
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace sph {
@@ -111,17 +113,19 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     // `n` inner entries (registers, then re-gathered beyond them); the ntot - n shell entries lie beyond
     // R_kern (1 + kShellEps) h0 and are only read while h exceeds kShellGrow h0 (exact: they contribute nothing below)
     const double hlim = kShellGrow * h0;
-    auto sums = [&](double hcur, double hinv, double& rho_sum, double& S) {
+    // (with_rho = false_type: the closing pass needs S only; the f polynomial then drops out at compile time)
+    auto sums = [&](auto with_rho, double hcur, double hinv, double& rho_sum, double& S) {
+        constexpr bool kRho = decltype(with_rho)::value;
         double rs = 0.0, ss = 0.0;
 #pragma unroll
         for (int c = 0; c < kRegChunksK<K>; ++c) {
             double f, g;
             kern_f_g<K>(r[c] * hinv, f, g);
             if (UNIM) {
-                rs += f;
+                if (kRho) rs += f;
                 ss += g;
             } else {
-                rs = fma(mb[c], f, rs);
+                if (kRho) rs = fma(mb[c], f, rs);
                 ss = fma(mb[c], g, ss);
             }
         }
@@ -131,7 +135,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
             double f, g;
             const double mm = UNIM ? 1.0 : sm[b];
             kern_f_g<K>(sep_r<WRAP>(xa, ya, za, sx, sy, sz, b, db) * hinv, f, g);
-            rs = fma(mm, f, rs);
+            if (kRho) rs = fma(mm, f, rs);
             ss = fma(mm, g, ss);
         }
         if (hcur > hlim) {
@@ -145,7 +149,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
                 ss = fma(mm, g, ss);
             }
         }
-        rs = octet_sum(rs);
+        if (kRho) rs = octet_sum(rs);
         ss = octet_sum(ss);
         const double c3 = (UNIM ? m0 : 1.0) * kern_cnorm(K) * hinv * hinv * hinv;
         rho_sum = c3 * rs;            // Eq. 1-2
@@ -159,7 +163,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     while (__any_sync(0xffffffffu, active)) {      // the four octets of a warp iterate together
         double rho_sum, S;
         const double hinv = 1.0 / h;                                // the one reciprocal of a sweep besides f / f'
-        sums(h, hinv, rho_sum, S);
+        sums(std::true_type{}, h, hinv, rho_sum, S);
         if (active) {
             ++it;
             const double hf = dp.hfact * hinv;
@@ -180,7 +184,7 @@ __device__ __forceinline__ void octet_solve(double xa, double ya, double za, dou
     }
     double rho_sum, S;
     const double hinv = 1.0 / h;
-    sums(h, hinv, rho_sum, S);
+    sums(std::false_type{}, h, hinv, rho_sum, S);      // closing pass at the converged h: Omega needs S only
     const double hf = dp.hfact * hinv;
     const double rho_a = ma * hf * hf * hf;
     out.h = h;
