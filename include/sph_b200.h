@@ -172,8 +172,11 @@ int sph_init_ex(sph_ctx** out, int64_t N, sph_mem mem, const double* pos, const 
  * the group-group criterion and the object-object criterion with radius
  * R_kern chi max(h_a,h_b) -> neighbour cache (the count / prefix / fill of Alg. 5, done per leaf
  * group in one pass: hits are buffered on chip, counted, space is taken from a bump allocator, lists written).
- * The cache is group-local: per group the array of candidate slots, per particle an ascending list of 16-bit
- * indices into it; sph_get_neighbours converts to a CSR over sorted slots.
+ * The cache is group-local: per group the array of candidate slots, per particle a list of 16-bit indices into it,
+ * inner entries first (d < R_kern 1.02 max(h_a, h_b) at build time), then the shell entries kept for the tolerance chi,
+ * which density and forces skip until some h has grown by 2 % (exact); sph_get_neighbours converts to
+ * a CSR over sorted slots. The pair test d^2 < (R_kern chi max(h_a, h_b))^2 is decided in packed fp32 wherever fp32 can
+ * decide it and re-decided in IEEE fp64 otherwise, so the sets are those of the fp64 definition.
  * Synchronises the stream once (reads the totals; repeats the pass with larger pools if one overflowed). */
 int sph_build_tree(sph_ctx* ctx);
 
