@@ -69,9 +69,9 @@ template <int HC>
 struct TravWarpSmemT {
     static constexpr int kCap = HC, kStride = HC + kHitSlack + 8;   // in u16; rows 16-byte aligned (copied out as uint4)
     uint32_t stack[kStackCap];
-    uint32_t plo[kPendCap], pn[kPendCap];     // pending buckets: first slot | wrap bit, particle count
+    uint32_t plo[kPendCap + 1], pn[kPendCap + 1];   // pending buckets: first slot | wrap bit, particle count (+ a sentinel)
     float prc[kPendCap];                      // their reach R_kern chi hmax_node in the group's scaled units, rounded up
-    float4 cand[kGroup + 2];                  // staged candidates (compacted), in pairs: {x0, x1, y0, y1}, {z0, z1, r0, r1}:
+    float4 cand[kGroup + 4];                  // staged candidates (compacted), in pairs: {x0, x1, y0, y1}, {z0, z1, r0, r1}:
                                               // scaled fp32 coordinates relative to the group's centre, r = cutoff^2
     uint32_t cslotb[kGroup];                  // their sorted slots (exact path)
     uint32_t ub[kUbCap];                      // bucket nodes within reach of the kShare groups' common box
@@ -250,7 +250,9 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
     const unsigned long long ax2 = pk2(G.ax, G.ax), ay2 = pk2(G.ay, G.ay), az2 = pk2(G.az, G.az);
     // software pipeline: the next bucket's candidate (one per lane) is in flight while this one is tested
     double px = 0.0, py = 0.0, pz = 0.0, ph = 0.0;
-    if (npend > 0) {
+    if (lane == 0) { s.plo[npend] = 0u; s.pn[npend] = 0u; }      // sentinel: the prefetch past the last bucket loads nothing
+    __syncwarp();
+    {
         const uint32_t blo = s.plo[0] & ~kWrapBit;
         if (lane < s.pn[0]) { px = x[blo + lane]; py = y[blo + lane]; pz = z[blo + lane]; ph = h[blo + lane]; }
     }
@@ -260,7 +262,7 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
         const bool wrap = (plo & kWrapBit) != 0u;
         G.anywrap |= wrap;
         const double cx = px, cy = py, cz = pz, ch = ph;
-        if (b + 1 < npend) {
+        {
             const uint32_t nlo = s.plo[b + 1] & ~kWrapBit;
             if (lane < s.pn[b + 1]) { px = x[nlo + lane]; py = y[nlo + lane]; pz = z[nlo + lane]; ph = h[nlo + lane]; }
         }
@@ -303,7 +305,7 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
             s.cslotb[pos] = blo + lane;
             if (DIRECT ? G.can_write : (G.ncs + pos < (uint32_t)kScrCap)) G.cptr[G.ncs + pos] = blo + lane;
         }
-        if (lane < 4u && nk + lane < ((nk + 3u) & ~3u)) {   // pad to a multiple of four with candidates nobody can hit
+        if (lane < 4u) {                                // four candidates nobody can hit behind the last one
             const uint32_t pp = nk + lane;
             float* q = cf + (pp >> 1) * 8 + (pp & 1u);
             q[0] = 1e18f; q[2] = 1e18f; q[4] = 1e18f; q[6] = 0.f;
@@ -366,8 +368,6 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
             asm volatile("" ::: "memory");
         }
         if (!DIRECT) {
-            G.nhit += ((wp - w0) + (q0 - wq)) >> 1;
-            G.nin += (wp - w0) >> 1;
             G.wpos = (wp - rowbase) >> 1;
             G.cpos = (rowtop - wq) >> 1;
             // A row keeps room for one more bucket only while it holds at most HC entries: when some lane is beyond
@@ -388,22 +388,22 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
                         for (uint32_t k = lane; k < cn; k += 32) dsc[k] = s.hits[p * S::kStride + (S::kCap + kHitSlack - cn) + k];
                     }
                     __syncwarp();
-                    G.nspill += G.wpos;
-                    G.cspill += G.cpos;
                 } else {
                     G.hard_overflow = true;       // the rows' content no longer matters, only the counts
                 }
+                G.nspill += G.wpos;
+                G.cspill += G.cpos;
                 G.wpos = 0u;
                 G.cpos = 0u;
                 wp = rowbase;
                 wq = rowtop;
             }
-        } else {
-            G.nhit = G.wpos + G.cpos;
-            G.nin = G.wpos;
         }
         G.ncs += nk;
     }
+    // exact counts so far: inner = spilled + in the row (DIRECT: written), all = inner + shell
+    G.nin = (DIRECT ? 0u : G.nspill) + G.wpos;
+    G.nhit = G.nin + (DIRECT ? 0u : G.cspill) + G.cpos;
 }
 
 // One node against the box / hmax of G: group-group criterion on the squared box-box gap under the
