@@ -38,7 +38,7 @@ KERNEL_NAMES = ("M4", "M5", "M6", "Wendland C2", "Wendland C4", "Wendland C6")  
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the committed ncu --set full capture of this
 # workload: NOT measured by this run (bench.py never runs under a profiler); only quoted when bench runs that workload
 NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_all.md"
-NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.54e9, "traverse": 4.71e9, "density": 5.10e9}
+NCU_TRAFFIC_BYTES_CUBE256 = {"forces": 6.54e9, "traverse": 4.71e9, "density": 5.10e9}   # profiles/r2_ncu_all.md rows 24, 19, 21
 
 
 def reduce_over_ranks(ms_local: float, n_local: float, world: int, device):
