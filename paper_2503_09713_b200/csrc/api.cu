@@ -156,7 +156,7 @@ static int grow_pool(sph_ctx* c, T** pool, uint64_t* cap, uint64_t want) {
     if (*pool) dfree(c, *pool);
     *pool = nullptr;
     *cap = 0;
-    SPH_TRY(dalloc(c, pool, (size_t)want));
+    SPH_TRY(dalloc(c, pool, (size_t)want + 64));   // 64 entries of slack: k_forces prefetches up to 15 list entries past a list's end
     *cap = want;
     return SPH_OK;
 }
