@@ -1,9 +1,13 @@
 // leapfrog.cu -- a7: leapfrog kick-drift-kick with a global timestep (G1-G5, order of
 // Fig. G1; u integrated like v, reading A13). Elementwise and HBM-bound. The timestep is
 // read from device memory so that a step needs no host round trip for dt (reading A14).
+#include <utility>
+
 #include "common.cuh"
 
 namespace sph {
+
+void adopt_new_acc(sph_ctx* c);
 
 struct WrapBox { double lo[3], hi[3], L[3]; int periodic[3]; };
 
@@ -42,8 +46,8 @@ __global__ void __launch_bounds__(256) k_predict(int64_t N, Fields f, WrapBox wb
     }
 }
 
-// G5: v = v* + dt/2 (a_new - a_old); then a_old <- a_new (same for u)
-// G5: v = v* + dt/2 (a_new - a_old); then a_old <- a_new (same for u). With ERR the kernel also reduces, per block
+// G5: v = v* + dt/2 (a_new - a_old) (same for u); a_old <- a_new is a swap of the two buffers on the host
+// (adopt_new_acc). With ERR the kernel also reduces, per block
 // and in a fixed order, the two quantities of the corrector check G6-G7 (reading A15):
 // max |dv|^2 and sum |v^{n+1}|^2.
 template <bool ERR>
@@ -56,10 +60,10 @@ __global__ void __launch_bounds__(256) k_correct(int64_t N, Fields f, const doub
     if (i < N) {
         const double hdt = 0.5 * *dtp;
         double a, dv, v;
-        a = nax[i]; dv = hdt * (a - f.ax[i]); v = f.vx[i] + dv; f.vx[i] = v; f.ax[i] = a; d2 = dv * dv; v2 = v * v;
-        a = nay[i]; dv = hdt * (a - f.ay[i]); v = f.vy[i] + dv; f.vy[i] = v; f.ay[i] = a; d2 += dv * dv; v2 += v * v;
-        a = naz[i]; dv = hdt * (a - f.az[i]); v = f.vz[i] + dv; f.vz[i] = v; f.az[i] = a; d2 += dv * dv; v2 += v * v;
-        a = ndu[i]; f.u[i] = f.u[i] + hdt * (a - f.du[i]); f.du[i] = a;
+        a = nax[i]; dv = hdt * (a - f.ax[i]); v = f.vx[i] + dv; f.vx[i] = v; d2 = dv * dv; v2 = v * v;
+        a = nay[i]; dv = hdt * (a - f.ay[i]); v = f.vy[i] + dv; f.vy[i] = v; d2 += dv * dv; v2 += v * v;
+        a = naz[i]; dv = hdt * (a - f.az[i]); v = f.vz[i] + dv; f.vz[i] = v; d2 += dv * dv; v2 += v * v;
+        a = ndu[i]; f.u[i] = f.u[i] + hdt * (a - f.du[i]);
     }
     if (ERR) {
         __shared__ double smax[8], ssum[8];
@@ -92,15 +96,6 @@ __global__ void __launch_bounds__(256) k_corr_final(int nblocks, const double* _
         __syncthreads();
     }
     if (threadIdx.x == 0) { sc->corr_dvmax2 = smax[0]; sc->corr_v2sum = ssum[0]; }
-}
-
-// copy a^{n+1} into the a^n slots without a velocity correction (white step)
-__global__ void __launch_bounds__(256) k_adopt_acc(int64_t N, Fields f, const double* __restrict__ nax,
-                                                   const double* __restrict__ nay, const double* __restrict__ naz,
-                                                   const double* __restrict__ ndu) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    f.ax[i] = nax[i]; f.ay[i] = nay[i]; f.az[i] = naz[i]; f.du[i] = ndu[i];
 }
 
 __global__ void __launch_bounds__(256) k_hmax(int64_t N, const double* __restrict__ h, DevScalars* sc) {
@@ -142,6 +137,7 @@ int launch_correct(sph_ctx* c, bool with_check) {
     }
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
+    adopt_new_acc(c);
     return SPH_OK;
 }
 
@@ -154,10 +150,14 @@ int launch_hmax(sph_ctx* c) {
     return SPH_OK;
 }
 
-int launch_adopt_acc(sph_ctx* c) {
-    k_adopt_acc<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, c->cur, c->nax, c->nay, c->naz, c->ndu);
-    c->launches++;
-    SPH_CUDA(c, cudaGetLastError());
+// a^n <- a^{n+1}, du/dt^n <- du/dt^{n+1}: the buffers change places (nothing is copied; stream order keeps every
+// kernel already enqueued on its own pointers)
+void adopt_new_acc(sph_ctx* c) {
+    std::swap(c->cur.ax, c->nax); std::swap(c->cur.ay, c->nay); std::swap(c->cur.az, c->naz);
+    std::swap(c->cur.du, c->ndu);
+}
+int launch_adopt_acc(sph_ctx* c) {      // white step / standalone force evaluation: no velocity correction
+    adopt_new_acc(c);
     return SPH_OK;
 }
 
