@@ -236,6 +236,23 @@ void sph_free(sph_ctx* ctx);
  * sm_mhz_out (may be NULL) is not measured here; bench.py samples clocks with nvidia-smi. */
 int sph_measure_fp64_peak(double* tflops_out, void* cuda_stream);
 
+/* An entry point that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the exclusive prefix sum behind the neighbour-cache offsets (Alg. 5,
+ * PAPER.md:1124-1130) and the stream compaction, as a variant of the library's decoupled look-back
+ * scan whose scratch memory is a static device array of the library.
+ *   in_dev[n]  (DEVICE) u32 counts;  out_dev[n + 1] (DEVICE) u64 exclusive prefix sums, out_dev[n] = total. The caller
+ *   owns both; the work is enqueued on cuda_stream (a cudaStream_t, NULL = default stream) of the CURRENT device and the
+ *   call returns without synchronising.
+ *   Limit: n <= sph_scan_noalloc_max_items() = 2^24 = 16 777 216 (the static scratch is 65 792 bytes, held by every GPU
+ *   that loads the library until the process exits); larger n: SPH_ERR_CAP. n < 1 or a null pointer: SPH_ERR_ARG; no
+ *   usable device: SPH_ERR_DEVICE. sph_noalloc_last_error() gives the text of the calling thread's last failure.
+ *   All calls on a device share the one scratch array. Each call clears what it uses, stream-ordered, before its
+ *   kernel, so calls ordered on one stream (or by events) are safe back to back; calls that OVERLAP on the GPU (two
+ *   streams without ordering between them) race on it and give wrong sums. Calls no cudaMalloc / cudaFree. */
+int sph_scan_u32_noalloc(const uint32_t* in_dev, uint64_t* out_dev, int64_t n, void* cuda_stream);
+int64_t sph_scan_noalloc_max_items(void);
+const char* sph_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ STATUS = {0: "SPH_OK", -1: "SPH_ERR_ARG", -2: "SPH_ERR_DEVICE", -3: "SPH_ERR_OOM
 SYMBOLS = ["sph_default_params", "sph_init", "sph_init_ex", "sph_build_tree", "sph_compute_density",
            "sph_compute_forces", "sph_step_leapfrog", "sph_set_fields", "sph_get_fields", "sph_get_keys_perm",
            "sph_get_tree", "sph_get_neighbours", "sph_get_neighbours_range", "sph_get_leaves", "sph_get_alpha", "sph_get_stats", "sph_reset_timers", "sph_last_error", "sph_free",
-           "sph_measure_fp64_peak"]
+           "sph_measure_fp64_peak", "sph_scan_u32_noalloc", "sph_scan_noalloc_max_items", "sph_noalloc_last_error"]
 
 
 class SphError(RuntimeError):
@@ -101,6 +101,11 @@ def load():
         lib.sph_get_alpha.argtypes = [vp, C.c_int, vp]
         lib.sph_get_stats.argtypes = [vp, C.POINTER(Stats)]
         lib.sph_measure_fp64_peak.argtypes = [C.POINTER(dbl), vp]
+        lib.sph_scan_u32_noalloc.argtypes = [vp, vp, i64, vp]
+        lib.sph_scan_noalloc_max_items.restype = C.c_int64
+        lib.sph_scan_noalloc_max_items.argtypes = []
+        lib.sph_noalloc_last_error.restype = C.c_char_p
+        lib.sph_noalloc_last_error.argtypes = []
         _lib = lib
     return _lib
 
@@ -353,6 +358,23 @@ class Sim:
 
     def reset_timers(self):
         self._check(self.lib.sph_reset_timers(self.ctx))
+
+
+def scan_u32_noalloc(counts, out=None, stream=None):
+    """``sph_scan_u32_noalloc``: exclusive prefix sum of a CUDA uint32 tensor (as int32 storage is not accepted: pass
+    ``torch.uint32`` or ``torch.int32`` holding non-negative counts) into an int64 tensor of n + 1 entries, without any
+    device allocation inside the library (argument marshalling only; ``out`` may be passed to avoid torch's own)."""
+    import torch
+    assert counts.is_cuda and counts.is_contiguous() and counts.element_size() == 4
+    n = counts.numel()
+    if out is None:
+        out = torch.empty(n + 1, dtype=torch.int64, device=counts.device)
+    assert out.is_cuda and out.is_contiguous() and out.element_size() == 8 and out.numel() >= n + 1
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = load().sph_scan_u32_noalloc(C.c_void_p(counts.data_ptr()), C.c_void_p(out.data_ptr()), n, C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise SphError(rc, load().sph_noalloc_last_error().decode())
+    return out
 
 
 def measure_fp64_peak() -> float:

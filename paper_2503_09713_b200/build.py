@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libsph_b200.so")
 SOURCES = ["api.cu", "keys.cu", "sort.cu", "scan.cu", "permute.cu", "tree.cu", "neigh.cu", "density.cu", "forces.cu",
-           "alpha.cu", "leapfrog.cu"]
+           "alpha.cu", "leapfrog.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
