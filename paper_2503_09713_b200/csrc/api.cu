@@ -156,7 +156,10 @@ static int grow_pool(sph_ctx* c, T** pool, uint64_t* cap, uint64_t want) {
     if (*pool) dfree(c, *pool);
     *pool = nullptr;
     *cap = 0;
-    SPH_TRY(dalloc(c, pool, (size_t)want + 64));   // 64 entries of slack: k_forces prefetches up to 15 list entries past a list's end
+    // slack behind the capacity: k_forces prefetches list entries unconditionally while ANY octet of its warp has entries
+    // left, so a lane with a short list reads up to (longest list of the warp + 15) entries past its own list's start;
+    // a list holds at most 65535 entries (16-bit candidate indices), which bounds the overrun behind the last list
+    SPH_TRY(dalloc(c, pool, (size_t)want + 65536 + 64));
     *cap = want;
     return SPH_OK;
 }
