@@ -70,7 +70,8 @@ struct TravWarpSmemT {
     static constexpr int kCap = HC, kStride = HC + kHitSlack + 8;   // in u16; rows 16-byte aligned (copied out as uint4)
     uint32_t stack[kStackCap];
     uint32_t plo[kPendCap + 1], pn[kPendCap + 1];   // pending buckets: first slot | wrap bit, particle count (+ a sentinel)
-    float prc[kPendCap];                      // their reach R_kern chi hmax_node in the group's scaled units, rounded up
+    float2 pkb[kPendCap + 1];                 // per pending bucket, from its reach and the group's (bucket_bounds): the prefilter's
+                                              // slack K and the fast path's uncertainty band B, in the group's scaled units
     float4 cand[kGroup + 4];                  // staged candidates (compacted), in pairs: {x0, x1, y0, y1}, {z0, z1, r0, r1}:
                                               // scaled fp32 coordinates relative to the group's centre, r = cutoff^2
     uint32_t cslotb[kGroup];                  // their sorted slots (exact path)
@@ -234,7 +235,7 @@ __device__ __forceinline__ void record_fast(GroupCtx& G, uint32_t& wp, uint32_t&
 // 1.19e-7), hence |d2_f - d2| <= 2 sqrt(3) E d + 3 E^2 + 3.01 2^-24 d2, the thresholds carry 2^-24 (query) and 3 2^-24
 // (candidate: (float)(R chi h s) squared) relative, and
 // for every test of a bucket  |v_f - v| <= B/4,  B := E (14 rcm' + 12 E) + 2.5e-6 rcm'^2,  v = d2 - max(cutoff^2),
-// rcm' = the larger of the query's and the bucket's reach (true hit: d <= rcm'; true miss: d2 - err(d) is increasing in
+// rcm' = the larger of the GROUP's and the bucket's reach, which bounds every query lane's (true hit: d <= rcm'; true miss: d2 - err(d) is increasing in
 // d beyond rcm', or E > rcm' / sqrt(3) and 12 E^2 covers it). So |v_f| > B implies sign(v_f) = sign(v), and sign(v) is
 // the fp64 decision because that differs from the real-number one only within 1e-15 relative of the cutoff.
 template <bool DIRECT, class S>
@@ -280,13 +281,10 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
             fx = (float)(rx * G.sc); fy = (float)(ry * G.sc); fz = (float)(rz * G.sc);
             fr = (float)(ch * G.ksc);                    // scaled cutoff radius, then its square: 3 roundings of 2^-24
             fr *= fr;
-            const float rcn = s.prc[b];
-            const float rcm_g = fmaxf(rcn, G.rcg);
-            const float E = 1.3e-7f * (G.twoA + 3.1f * rcm_g);
+            const float2 kb = s.pkb[b];                  // K = 16 E (rcm + E), B = E (14 rcm + 12 E) + 2.5e-6 rcm^2
             const float gx = fmaxf(fabsf(fx) - G.ex, 0.f), gy = fmaxf(fabsf(fy) - G.ey, 0.f), gz = fmaxf(fabsf(fz) - G.ez, 0.f);
-            keep = keep && (gx * gx + gy * gy + gz * gz <= fmaxf(fr, G.rc2g_f) * 1.0001f + 16.f * E * (rcm_g + E));
-            const float rcm = fmaxf(G.rca, rcn);
-            band = E * (14.f * rcm + 12.f * E) + 2.5e-6f * rcm * rcm;
+            keep = keep && (gx * gx + gy * gy + gz * gz <= fmaxf(fr, G.rc2g_f) * 1.0001f + kb.x);
+            band = kb.y;
         } else if (keep && !wrap) {   // plain fp64 version (groups too large for the scaled frame); wrapping buckets keep all
             const double rc = __dmul_rn(rk_chi, ch);
             const double rc2 = __dmul_rn(rc, rc);
@@ -406,6 +404,15 @@ __device__ __forceinline__ void stage2(S& s, GroupCtx& G, int npend, unsigned la
     G.nhit = G.nin + (DIRECT ? 0u : G.cspill) + G.cpos;
 }
 
+// The two error-bound terms of a bucket on the fp32 fast path (derivation above stage2), computed once per bucket by the
+// lane that found it: with rcm = the larger reach of the GROUP and the bucket (>= the rcm' of any query lane of the
+// group, so the band is the same or wider than the per-lane one: conservative) and E = 1.3e-7 (2 A + 3.1 rcm).
+__device__ __forceinline__ float2 bucket_bounds(float prc, const GroupCtx& G) {
+    const float rcm = fmaxf(prc, G.rcg);
+    const float E = 1.3e-7f * (G.twoA + 3.1f * rcm);
+    return make_float2(16.f * E * (rcm + E), E * (14.f * rcm + 12.f * E) + 2.5e-6f * rcm * rcm);
+}
+
 // One node against the box / hmax of G: group-group criterion on the squared box-box gap under the
 // minimum image, conservative under rounding (tiny pad); `wrap` says whether any (query, candidate) separation can
 // exceed L/2 on a periodic axis (exact: rounding is monotone). Entry e = internal node index, or leaf slot | kLeafBit.
@@ -505,7 +512,7 @@ __device__ __forceinline__ void refine(S& s, GroupCtx& G, int nu, unsigned lane,
             const int at = nb + __popc(em & lt);
             s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
             s.pn[at] = r.rhi - r.rlo + 1;
-            s.prc[at] = r.prc;
+            s.pkb[at] = bucket_bounds(r.prc, G);
         }
         nb += __popc(em);
         __syncwarp();
@@ -549,7 +556,7 @@ __device__ __forceinline__ void walk(S& s, GroupCtx& G, unsigned lane, unsigned 
             const int at = nb + __popc(em & lt);
             s.plo[at] = r.rlo | (r.wrap ? kWrapBit : 0u);
             s.pn[at] = r.rhi - r.rlo + 1;
-            s.prc[at] = r.prc;
+            s.pkb[at] = bucket_bounds(r.prc, G);
         }
         nb += __popc(em);
         __syncwarp();
