@@ -126,17 +126,30 @@ __global__ void __launch_bounds__(256) k_aabb_groups(int64_t N, const double* __
             srcL = mine ? (int)(split - (int64_t)glo) : 0;
             srcR = mine ? srcL + 1 : 0;
         }
-        double b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0, b4 = 0.0, b5 = 0.0, b6 = 0.0;   // my node: lo xyz, hi xyz, hmax
-        bool done = !mine;
-        for (;;) {
-            const unsigned dm = __ballot_sync(0xffffffffu, done);
-            if (dm == 0xffffffffu) break;
-            const bool ok = !done && (lleaf || ((dm >> srcL) & 1u)) && (rleaf || ((dm >> srcR) & 1u));
-            // children: a leaf's box is its position, an internal child's box is that lane's node
+        // my node: lo xyz, hi xyz, hmax. Leaf children first (one exchange of the leaves' positions), then rounds over
+        // the internal children only: a child whose node is complete hands its box over by shuffles. min / max by
+        // compare-and-select (no NaNs here; fmin / fmax expand to NaN-safe sequences); they are exact, so the order in
+        // which the two children are merged does not matter.
+        auto mn = [](double a, double b) { return a < b ? a : b; };
+        auto mx = [](double a, double b) { return a > b ? a : b; };
+        const double inf = __longlong_as_double(0x7ff0000000000000ll);
+        double b0 = inf, b1 = inf, b2 = inf, b3 = -inf, b4 = -inf, b5 = -inf, b6 = 0.0;
+        {
             const double Llx = __shfl_sync(0xffffffffu, lx, srcL), Lly = __shfl_sync(0xffffffffu, ly, srcL);
             const double Llz = __shfl_sync(0xffffffffu, lz, srcL), Llh = __shfl_sync(0xffffffffu, lh, srcL);
             const double Rlx = __shfl_sync(0xffffffffu, lx, srcR), Rly = __shfl_sync(0xffffffffu, ly, srcR);
             const double Rlz = __shfl_sync(0xffffffffu, lz, srcR), Rlh = __shfl_sync(0xffffffffu, lh, srcR);
+            if (mine && lleaf) { b0 = Llx; b1 = Lly; b2 = Llz; b3 = Llx; b4 = Lly; b5 = Llz; b6 = Llh; }
+            if (mine && rleaf) {
+                b0 = mn(b0, Rlx); b1 = mn(b1, Rly); b2 = mn(b2, Rlz); b3 = mx(b3, Rlx); b4 = mx(b4, Rly); b5 = mx(b5, Rlz);
+                b6 = mx(b6, Rlh);
+            }
+        }
+        bool needL = mine && !lleaf, needR = mine && !rleaf;
+        for (;;) {
+            const unsigned dm = __ballot_sync(0xffffffffu, !needL && !needR);      // complete nodes (and idle lanes)
+            if (dm == 0xffffffffu) break;
+            const bool okL = needL && ((dm >> srcL) & 1u), okR = needR && ((dm >> srcR) & 1u);
             const double L0 = __shfl_sync(0xffffffffu, b0, srcL), L1 = __shfl_sync(0xffffffffu, b1, srcL);
             const double L2 = __shfl_sync(0xffffffffu, b2, srcL), L3 = __shfl_sync(0xffffffffu, b3, srcL);
             const double L4 = __shfl_sync(0xffffffffu, b4, srcL), L5 = __shfl_sync(0xffffffffu, b5, srcL);
@@ -145,12 +158,15 @@ __global__ void __launch_bounds__(256) k_aabb_groups(int64_t N, const double* __
             const double R2 = __shfl_sync(0xffffffffu, b2, srcR), R3 = __shfl_sync(0xffffffffu, b3, srcR);
             const double R4 = __shfl_sync(0xffffffffu, b4, srcR), R5 = __shfl_sync(0xffffffffu, b5, srcR);
             const double R6 = __shfl_sync(0xffffffffu, b6, srcR);
-            if (ok) {
-                b0 = fmin(lleaf ? Llx : L0, rleaf ? Rlx : R0); b1 = fmin(lleaf ? Lly : L1, rleaf ? Rly : R1);
-                b2 = fmin(lleaf ? Llz : L2, rleaf ? Rlz : R2); b3 = fmax(lleaf ? Llx : L3, rleaf ? Rlx : R3);
-                b4 = fmax(lleaf ? Lly : L4, rleaf ? Rly : R4); b5 = fmax(lleaf ? Llz : L5, rleaf ? Rlz : R5);
-                b6 = fmax(lleaf ? Llh : L6, rleaf ? Rlh : R6);
-                done = true;
+            if (okL) {
+                b0 = mn(b0, L0); b1 = mn(b1, L1); b2 = mn(b2, L2); b3 = mx(b3, L3); b4 = mx(b4, L4); b5 = mx(b5, L5);
+                b6 = mx(b6, L6);
+                needL = false;
+            }
+            if (okR) {
+                b0 = mn(b0, R0); b1 = mn(b1, R1); b2 = mn(b2, R2); b3 = mx(b3, R3); b4 = mx(b4, R4); b5 = mx(b5, R5);
+                b6 = mx(b6, R6);
+                needR = false;
             }
         }
         if (mine) {
