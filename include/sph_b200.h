@@ -132,8 +132,8 @@ typedef struct {
   int32_t groups_fallback; /* groups that overflowed their buffers and were walked a second time          */
   int32_t chunks_shared;   /* chunks of consecutive groups that shared one tree walk (0: sharing off)     */
   int32_t share_chunk;     /* groups per chunk used by the last pass (1 or 4)                             */
-  int32_t sort_passes;     /* radix passes of the last sort: 8, or 5 in prefix mode (top 40 bits + tie repair) */
-  int32_t sort_tie_max;    /* longest run of keys equal in their top 40 bits seen by the last sort         */
+  int32_t sort_passes;     /* radix passes of the last sort: 8, or 5 / 4 in prefix mode (top 40 / 32 bits + tie repair) */
+  int32_t sort_tie_max;    /* longest run of keys equal in their top 40 bits (32 after a 4-pass sort) seen by the last sort */
   int32_t recycles;        /* corrector re-cycles of the last step (eps_v > 0)                              */
   int32_t reserved;
   double cfl_mult;         /* CFL multiplier lambda_CFL applied to the next internal dt                     */

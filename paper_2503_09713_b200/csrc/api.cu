@@ -187,7 +187,13 @@ static int cache_build(sph_ctx* c) {
             fprintf(stderr, "[sph] groups %u nc_max %u fallback %u nbr_min %u nbr_max %u lists %llu candidates %llu chunk %u shared %u overflow %u\n",
                     s.n_groups, s.nc_max, s.n_fallback, s.nbr_min, s.nbr_max, s.list_cursor, s.cslot_cursor, c->last_chunk,
                     s.n_chunks_shared, s.n_chunks_overflow);
-        c->sort_p0 = (s.tie_max <= 64u && !getenv("SPH_FULL_SORT")) ? 3 : 0;   // next sort: prefix mode if ties stay short
+        // next sort: prefix mode if ties stay short -- four passes (top 32 bits) if the runs of equal 32-bit prefixes are
+        // short, else five (top 40 bits) if those are; a four-pass sort has no 40-bit census: it is followed by a
+        // five-pass one when its own runs got long (the repair kernel's bound and the redo path guard that sort too)
+        if (getenv("SPH_FULL_SORT")) c->sort_p0 = 0;
+        else if (s.tie_max32 <= 64u) c->sort_p0 = 4;
+        else if (c->last_sort_passes == 4 || s.tie_max <= 64u) c->sort_p0 = 3;
+        else c->sort_p0 = 0;
         if (c->last_chunk > 1) {
             const uint64_t chunks = ((uint64_t)s.n_groups + c->last_chunk - 1) / c->last_chunk;
             if ((uint64_t)s.n_chunks_shared * 10 < chunks * 8 || (uint64_t)s.n_chunks_overflow * 50 > chunks)
@@ -699,7 +705,8 @@ int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->kernel_launches = c->launches; out->dt = c->cfl_mult * s.dt; out->t = s.t; out->bytes_allocated = c->bytes_allocated;
     out->cand_max = (int32_t)s.nc_max; out->groups_fallback = (int32_t)s.n_fallback;
     out->chunks_shared = (int32_t)s.n_chunks_shared; out->share_chunk = (int32_t)c->last_chunk;
-    out->sort_passes = c->last_sort_passes; out->sort_tie_max = (int32_t)s.tie_max;
+    out->sort_passes = c->last_sort_passes;
+    out->sort_tie_max = (int32_t)(c->last_sort_passes == 4 ? s.tie_max32 : s.tie_max);
     out->recycles = c->recycles_last; out->cfl_mult = c->cfl_mult; out->density_sweeps = (int64_t)s.sweeps; out->n_inner = (int64_t)s.n_inner; out->n_grew = (int64_t)s.n_grew;
     return SPH_OK;
 }

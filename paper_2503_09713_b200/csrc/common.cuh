@@ -83,6 +83,7 @@ struct DevScalars {
     unsigned int n_chunks_overflow;
     double corr_dvmax2, corr_v2sum;  // corrector check G7: max |dv|^2, sum |v|^2 (reading A15)
     unsigned int tie_max;            // longest run of keys equal in their top 40 bits (sort prefix mode)
+    unsigned int tie_max32;          // the same for the top 32 bits (runs longer than 65 are reported as 66)
     unsigned int mass_nonuniform;    // set at init if any two particle masses differ
     unsigned int n_fallback;         // groups that took the two-walk fallback (hit or bucket buffer overflow)
     unsigned int sort_redo;          // prefix-mode sort met a run of equal prefixes too long to repair: the tree kernels
@@ -171,7 +172,8 @@ struct sph_ctx {
     double cfl_mult = 1.0;              // CFL multiplier lambda_CFL (G9-G10)
     int recycles_last = 0;              // corrector re-cycles of the last step
     int last_sort_passes = 8;
-    int sort_p0 = 0;                    // first radix pass: 0 = all eight passes, 3 = prefix mode (top 40 bits + repair)
+    int sort_p0 = 0;                    // first radix pass: 0 = all eight passes; prefix modes: 3 = top 40 bits + repair,
+                                        // 4 = top 32 bits + repair
     bool share_disabled = false;        // traversal: shared walks switched off (too few chunks could share)
     uint32_t last_chunk = 1;
     bool uniform_mass = false;          // all particle masses equal (density kernel variant)

@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ 
 
 // ---- kernel 2: exclusive scan of each digit histogram -> global digit bases ----
 __global__ void __launch_bounds__(kRadix) k_sort_bases(uint32_t* __restrict__ ghist, DevScalars* sc) {
-    if (threadIdx.x == 0) { sc->tie_max = 0u; sc->sort_redo = 0u; }
+    if (threadIdx.x == 0) { sc->tie_max = 0u; sc->tie_max32 = 0u; sc->sort_redo = 0u; }
     __shared__ uint32_t wsum[kRadix / 32];
     const unsigned d = threadIdx.x, lane = lane_id(), w = d >> 5;
     for (int p = 0; p < kPasses; ++p) {
@@ -252,16 +252,28 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_onesweep(const uint64_t* __
 // raises sc->sort_redo instead, the tree kernels of this build then do nothing, and the host sorts again with all
 // eight passes (api.cu). Prefix mode is only chosen after a sort whose longest run was <= 64, so this needs a sudden
 // collapse of many particles into one 2^-13 cell between two steps.
+// Two prefix lengths: 40 bits (shift 24, five passes) and 32 bits (shift 32, four passes: cells of 2^-10.7 of the box
+// per axis, enough wherever the particle spacing is a few times that). The census is taken for both: at shift 24 the
+// kernel also measures the runs of equal 32-bit prefixes (bounded walks; repairs inside 40-bit runs leave the top 40
+// bits of every position unchanged, so this may read while other threads repair), at shift 32 its runs are those.
 __global__ void __launch_bounds__(256) k_sort_repair(int64_t N, uint64_t* __restrict__ key, uint32_t* __restrict__ val,
                                                      int shift, int64_t max_run, DevScalars* sc) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    if (shift < 32) {
+        const uint64_t p32 = key[i] >> 32;
+        if (i == 0 || (key[i - 1] >> 32) != p32) {
+            int64_t e = i + 1;
+            while (e < N && e - i <= 65 && (key[e] >> 32) == p32) ++e;
+            if (e - i >= 2) atomicMax(&sc->tie_max32, (unsigned int)(e - i));
+        }
+    }
     const uint64_t p = key[i] >> shift;
     if (i > 0 && (key[i - 1] >> shift) == p) return;          // not the head of a run
     int64_t e = i + 1;
     while (e < N && e - i <= max_run && (key[e] >> shift) == p) ++e;
     if (e - i < 2) return;
-    atomicMax(&sc->tie_max, (unsigned int)min(e - i, (int64_t)0x7fffffff));
+    atomicMax(shift < 32 ? &sc->tie_max : &sc->tie_max32, (unsigned int)min(e - i, (int64_t)0x7fffffff));
     if (e - i > max_run) { sc->sort_redo = 1u; return; }
     for (int64_t a = i + 1; a < e; ++a) {
         const uint64_t kk = key[a];
@@ -290,8 +302,8 @@ int launch_sort(sph_ctx* c) {
     SPH_CUDA(c, cudaMemsetAsync(c->sort_status, 0, kPasses * status_per_pass * sizeof(uint32_t), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(c->sort_counters, 0, kPasses * sizeof(uint32_t), c->stream));
     unsigned hb = (unsigned)min((int64_t)148 * 8, (N + 255) / 256);
-    // Prefix mode: sort on the top 40 bits only (five passes) and repair the rare runs of equal prefixes; chosen by
-    // the host from the longest run seen in the previous sort (api.cu), all eight passes otherwise.
+    // Prefix mode: sort on the top 40 or 32 bits only (five or four passes) and repair the rare runs of equal prefixes;
+    // chosen by the host from the longest runs seen in the previous sort (api.cu), all eight passes otherwise.
     // morton_bits = 10: the code sits in bits 62..33, four passes (bits 32..63) sort it completely, no repair
     const bool short_codes = c->p.morton_bits == 10;
     const int p0 = short_codes ? 4 : c->sort_p0;
@@ -318,7 +330,7 @@ int launch_sort(sph_ctx* c) {
         // SPH_REPAIR_MAX (tests) lowers the bound so that the redo path can be reached with small inputs
         const char* env = getenv("SPH_REPAIR_MAX");
         const int64_t max_run = (p0 == 0) ? (int64_t)1 << 40 : (env ? (int64_t)atoll(env) : kRepairMaxRun);
-        k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, kPrefixShift, max_run, c->d_sc);
+        k_sort_repair<<<div_up(N, 256), 256, 0, c->stream>>>(N, c->key, c->val, p0 == 4 ? 32 : kPrefixShift, max_run, c->d_sc);
         c->launches++;
     }
     SPH_CUDA(c, cudaGetLastError());

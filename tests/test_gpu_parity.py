@@ -497,7 +497,7 @@ def _stepped_parity(w, sim, n_steps, check_steps, blocks, count=1024, tree=True,
 def test_c2_full_size_stepped_parity():
     """BASELINE config 2 at full size (256^3 = 16.8 M particles), the workload and launch configuration bench.py
     times, for its 5 steps. White step: integer stages bit-exact on all particles, sampled parity (interior; across the
-    periodic corner) and neighbour sets on Morton blocks. After steps 2 and 5 (five-pass prefix sort + repair, reused
+    periodic corner) and neighbour sets on Morton blocks. After steps 2 and 5 (prefix sort + repair, reused
     pools, shared walks): the same, from the GPU's own pre-step state (P1)."""
     w = W.cube(256, jitter=0.1, steps=5)
     box, p = O.workload_box_params(w)
@@ -514,7 +514,7 @@ def test_c2_full_size_stepped_parity():
     assert st["n_groups"] == w.n // 32 and 75 < st["nbr_mean"] < 90
     del f, gperm
     st = _stepped_parity(w, sim, 5, (2, 5), (0.0, 0.37, 0.999))
-    assert st["sort_passes"] == 5 and st["share_chunk"] == 4     # the configuration the bench times
+    assert st["sort_passes"] == 4 and st["share_chunk"] == 4     # the configuration the bench times (32-bit prefix sort)
     _invariants(w, sim)
     sim.close()
 
@@ -724,8 +724,9 @@ def _check_sorted_state(sim, pos, box, prev_perm=None):
 
 @pytest.mark.parametrize("cluster", [24, 200], ids=["short_runs_prefix_mode", "long_runs_full_sort"])
 def test_sort_prefix_mode_and_tie_repair(cluster):
-    """From the second build on the sort uses five passes over the top 40 key bits plus a repair of the runs that
-    share them, if the previous sort saw only short runs (<= 64), else all eight passes. Clusters of particles
+    """From the second build on the sort uses four passes over the top 32 key bits (five over the top 40 if the 32-bit
+    runs are long) plus a repair of the runs that share them, if the previous sort saw only short runs (<= 64), else
+    all eight passes. Clusters of particles
     inside one 2^-14 cell make such runs; both modes must give the stable sort by the full key. The particles are
     moved by a ballistic leapfrog step (sph_set_fields with new positions goes back to the full sort)."""
     from paper_2503_09713_b200 import binding as B
@@ -756,7 +757,7 @@ def test_sort_prefix_mode_and_tie_repair(cluster):
     perm0 = sim.get_keys_perm()[1]
     sim.step_leapfrog(dt=1.0)
     st = sim.stats()
-    assert st["sort_passes"] == (5 if cluster <= 64 else 8) and st["sort_tie_max"] >= cluster
+    assert st["sort_passes"] == (4 if cluster <= 64 else 8) and st["sort_tie_max"] >= cluster
     pos_now = _np(sim.get_fields(("pos",)))["pos"]
     assert np.max(np.abs(pos_now - pos1)) < 1e-15
     _check_sorted_state(sim, pos_now, box, prev_perm=perm0)
@@ -784,7 +785,7 @@ def test_long_run_conservation_and_reproducibility():
         return f0, f, st
 
     f0, f, st = run()
-    assert st["steps"] == 40 and st["sort_passes"] == 5 and st["restarts"] == 0
+    assert st["steps"] == 40 and st["sort_passes"] == 4 and st["restarts"] == 0
     e0 = (w.mass * (0.5 * (f0["vel"] ** 2).sum(axis=0) + f0["u"])).sum()
     e1 = (w.mass * (0.5 * (f["vel"] ** 2).sum(axis=0) + f["u"])).sum()
     assert abs(e1 / e0 - 1) < 1e-5
@@ -1059,3 +1060,36 @@ def test_shock_switch_constant_alpha_limit():
     for k in ("pos", "vel", "u", "acc", "dudt"):
         assert np.allclose(fa[k], fb[k], rtol=1e-12, atol=1e-14 * np.abs(fa[k]).max()), k
     a.close(); b.close()
+
+
+def test_sort_prefix_lengths_follow_the_census():
+    """The prefix sort picks its length from the previous sort's census: 32 bits (four passes) where the runs of equal
+    32-bit prefixes are short, 40 bits (five passes) where only those are, all eight passes otherwise. Clusters of 100
+    particles spread over 3e-4 of the box share their top 32 key bits (cells of 6e-4) but not their top 40 (cells of
+    1e-4): five passes; each time the result is the stable sort by the full key."""
+    from paper_2503_09713_b200 import binding as B
+    n, ncl, cluster = 6000, 10, 100
+    w = W.random_cloud(n, seed=37, periodic=False, clustered=False)
+    w.h0 = np.minimum(w.h0, 0.1)
+    rng = np.random.default_rng(3)
+    cell = 2.0 ** -10                                            # cluster inside one 32-bit cell (2^-10.67 ... per axis >= 2^-11)
+    for c in range(ncl):
+        corner = np.floor(w.pos[:, c * cluster] / cell) * cell
+        w.pos[:, c * cluster:(c + 1) * cluster] = corner[:, None] + 0.45 * cell * rng.random((3, cluster)) + 0.02 * cell
+    w.pos = np.clip(w.pos, 0.0, np.nextafter(1.0, 0.0))
+    box, p = O.workload_box_params(w)
+    key = O.morton_keys(w.pos, box)
+    runs32 = np.unique(key >> np.uint64(32), return_counts=True)[1].max()
+    runs40 = np.unique(key >> np.uint64(24), return_counts=True)[1].max()
+    assert runs32 > 64 and runs40 <= 64                        # the input is what the docstring says
+    sim = _sim(w, params=B.params_for(w, max_h_iter=400))
+    assert sim.stats()["sort_passes"] == 8
+    seen = []
+    for _ in range(3):
+        perm0 = sim.get_keys_perm()[1]
+        sim.step_leapfrog(dt=1e-7)                               # positions all but unchanged
+        seen.append(sim.stats()["sort_passes"])
+        pos_now = _np(sim.get_fields(("pos",)))["pos"]
+        _check_sorted_state(sim, pos_now, box, prev_perm=perm0)
+    assert seen == [5, 5, 5]
+    sim.close()
